@@ -1,0 +1,194 @@
+/*
+ * spf.h -- C ABI of libspf: the M-TIP slicing + orientation-matching hot path on one B200.
+ *
+ * What the calls compute is fixed by the paper's problem statement (arxiv 2109.05339,
+ * /root/reference/PAPER.md; citations "PAPER.md:<line>"), the call names by
+ * BASELINE.json:north_star, and everything the paper leaves open by the readings in
+ * DESIGN.md ("Readings", s1..s15 of SURVEY.md section 8(c)).
+ *
+ *   spf_prepare_model  -- once per model update: deapodise, zero-pad to the upsampled grid,
+ *                         3-D FFT (steps a1-a2 of a type-2 NUFFT, refs [8],[15]).
+ *   spf_slice          -- M model images: rotate the detector pixels' q-vectors by each
+ *                         reference orientation and interpolate the upsampled grid there with
+ *                         the exponential-of-semicircle kernel (steps a3-a5).
+ *   spf_match          -- every image against every model image by squared Euclidean distance,
+ *                         argmin orientation per image (steps a6-a8).
+ *   spf_orientation_match_host -- the same three steps behind HOST buffers (what a user with
+ *                         NumPy arrays calls; bench.py's end-to-end number).
+ *
+ * Conventions
+ *   - Pointers marked [dev] are DEVICE pointers owned by the caller (allocate them with
+ *     PyTorch or cudaMalloc); [host] are host pointers.  Inputs are never modified, outputs are
+ *     fully overwritten.  The library owns only what lives inside its context (the fine grid,
+ *     deapodisation tables, cuFFT plan, tensor maps).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *     calls enqueue on it and return without synchronising, except where stated.
+ *   - Return value: SPF_OK (0) or a negative spf_status; spf_last_error() gives the text (for
+ *     SPF_ECUDA the CUDA error string).  No exception or abort crosses the ABI.
+ *   - There is no CPU fallback: without a CUDA device every call except spf_version /
+ *     spf_status_string / spf_plan_* fails with SPF_ECUDA.
+ *   - Layouts are C-order (last index fastest).  Model axes (x,y,z) = (i1,i2,i3); voxel
+ *     [i1][i2][i3] sits at integer position n = (i1,i2,i3) - floor(N/2)   (reading s1/s13).
+ *   - Quaternions are (w,x,y,z), Hamilton, active: x = R(quat) q; they are normalised inside
+ *     (reading s2).  q and -q give the same slice.
+ *   - Pixel q-vectors are in radians per voxel, |component| <= pi (values outside are folded
+ *     by 2 pi, the transform being 2 pi-periodic)   (reading s4).
+ */
+#ifndef SPF_H_
+#define SPF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define SPF_API __attribute__((visibility("default")))
+#else
+#define SPF_API
+#endif
+
+typedef enum {
+    SPF_OK = 0,
+    SPF_EINVAL = -1, /* bad size, null pointer, unsupported parameter (checked on host-side arguments only) */
+    SPF_ENOMEM = -2, /* host or device allocation failed */
+    SPF_ECUDA = -3,  /* a CUDA / cuFFT / driver call failed; text in spf_last_error */
+    SPF_ESTATE = -4  /* call order: spf_slice before spf_prepare_model */
+} spf_status;
+
+typedef struct spf_ctx spf_ctx; /* opaque */
+
+typedef struct {
+    int32_t n;        /* model edge N >= 2 (odd or even) */
+    double eps;       /* NUFFT tolerance in (0, 1e-1]; sets the kernel width w = ceil(log10(1/eps)) + 1, 2 <= w <= 16 */
+    double upsampfac; /* sigma >= 2.0 (the kernel constants are those of sigma = 2)        (reading s10) */
+    int32_t n_fine;   /* 0: smallest even 2-3-5-7-smooth integer >= upsampfac * n; else an explicit fine-grid edge >= 2n */
+    int32_t device;   /* CUDA device ordinal */
+} spf_params;
+
+typedef struct {
+    int32_t n, n_fine, w;   /* model edge, fine-grid edge actually used, kernel width in fine cells */
+    double beta;            /* exponential-of-semicircle shape parameter, 2.30 * w */
+    int32_t n_padded;       /* edge of the stored, centred fine grid including its periodic halo */
+    int32_t grid_is_real;   /* 1 after spf_prepare_model saw a real EVEN model (fine grid real; fp32 grid is gathered) */
+    int32_t prepared;       /* 1 once spf_prepare_model has run */
+    int32_t sm_count;       /* multiprocessors of the device */
+} spf_info;
+
+SPF_API const char *spf_version(void);
+SPF_API const char *spf_status_string(int status);
+
+/* Host-only planning helpers (no device needed): kernel width for eps, default fine-grid edge. */
+SPF_API int32_t spf_plan_kernel_width(double eps);
+SPF_API int32_t spf_plan_n_fine(int32_t n, double upsampfac);
+
+/*
+ * Create a context on p->device: allocates the fine grids (n_padded^3 complex64 + fp32),
+ * plans cuFFT, computes the deapodisation factors p(n) = 2 / (w phihat(pi w n / n_fine)) on the
+ * host in fp64 by Gauss-Legendre quadrature.  Synchronises the device.  *out = NULL on error
+ * (then spf_last_error(NULL) holds the text).
+ */
+SPF_API int spf_create(spf_ctx **out, const spf_params *p);
+SPF_API void spf_destroy(spf_ctx *ctx);
+SPF_API int spf_get_info(const spf_ctx *ctx, spf_info *out);
+SPF_API const char *spf_last_error(const spf_ctx *ctx); /* ctx may be NULL: error of the last failed spf_create */
+
+/*
+ * Optional layout promise that lets spf_slice bin points without a sort: the pixel array given
+ * to spf_slice is [n_panels][rows][cols][3], each panel a regular lattice (PAPER.md:124:
+ * "128 x 128 pixels").  Thread blocks then take compact lattice patches whose fine-grid
+ * bounding box is staged in shared memory.  Without the promise (n_panels = 0) blocks take
+ * runs of consecutive pixels: same results, lower locality.  Host-only state; returns EINVAL
+ * for non-positive sizes.
+ */
+SPF_API int spf_set_detector_layout(spf_ctx *ctx, int32_t n_panels, int32_t rows, int32_t cols);
+
+/*
+ * Steps a1-a2.  model [dev]: [n][n][n] real fp32.  Multiplies by the separable deapodisation
+ * factors, scatters into the zeroed n_fine^3 complex grid at index n mod n_fine, runs one
+ * forward (exponent -i, reading s1) 3-D cuFFT, and re-lays the result out centred with a
+ * periodic halo of ceil(w/2)+1 cells.  Also tests whether the model is exactly even
+ * (A[n] == A[-n]); if so the imaginary part of the grid is identically zero up to round-off and
+ * a real fp32 copy is what spf_slice gathers.  SYNCHRONISES `stream` once to read that flag
+ * back (this call is once per model update and is timed separately).
+ */
+SPF_API int spf_prepare_model(spf_ctx *ctx, const float *model, void *stream);
+
+#define SPF_OUT_COMPLEX 0   /* out: complex64 [M][P] (re, im interleaved), c_{m,j} */
+#define SPF_OUT_INTENSITY 1 /* out: fp32 [M][P], scale * Re c_{m,j}   (reading s3: a model image is Re c) */
+
+/*
+ * Steps a3-a5.  quats [dev] [M][4] fp32, pix_q [dev] [P][3] fp32, out [dev] per out_kind.
+ *   c_{m,j} ~= sum_n A[n] exp(-i n . R(quat_m) q_j)   to the NUFFT tolerance eps.
+ * M, P >= 0 (zero sizes are a no-op).  SPF_ESTATE before spf_prepare_model.
+ */
+SPF_API int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const float *pix_q, int64_t P, int32_t out_kind,
+                      float scale, void *out, void *stream);
+
+/*
+ * Steps a6-a8.  images [dev] [n_img][P] fp32, slices [dev] [M][P] fp32, mask [dev] [P] bytes
+ * (1 = use, 0 = leave the pixel out of every sum; NULL = all used; reading s8),
+ * best_idx [dev] [n_img] int32, best_dist [dev] [n_img] fp32,
+ * workspace [dev]: at least spf_match_workspace_bytes(n_img, M, P) bytes, 1024-byte aligned.
+ *   d_{i,m} = sum_{j: mask_j} (I_ij - S_mj)^2,  best_idx[i] = argmin_m d_{i,m} (lowest m on
+ *   exact ties of the computed fp32 distances), best_dist[i] = that distance.
+ * Evaluated as ||I||^2 + ||S||^2 - 2 I.S with the cross term on the tensor cores from
+ * two-term fp16 splits of both operands (fp32-equivalent products, fp32 accumulation); the
+ * distance matrix is never written to memory.  Requires M >= 1 when n_img >= 1.
+ * Values must satisfy |x| < 2^100 (they are rescaled by powers of two into fp16 range).
+ */
+SPF_API int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P,
+                      const uint8_t *mask, int32_t *best_idx, float *best_dist, void *workspace,
+                      size_t workspace_bytes, void *stream);
+SPF_API size_t spf_match_workspace_bytes(int64_t n_img, int64_t M, int64_t P);
+
+/*
+ * Debug variant of spf_match for tests: additionally writes the full distance matrix
+ * dist [dev] [n_img][M] fp32 with a plain CUDA-core kernel (difference form, fp32) -- used to
+ * check the tensor-core path from a second, independent GPU computation.  Small sizes only.
+ */
+SPF_API int spf_match_reference(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M,
+                                int64_t P, const uint8_t *mask, int32_t *best_idx, float *best_dist, float *dist,
+                                void *stream);
+
+/*
+ * The whole path behind HOST buffers (all pointers [host]; pinned memory makes the copies
+ * asynchronous): uploads model / quats / pix_q / images / mask, runs prepare -> slice -> match,
+ * downloads best_idx / best_dist, synchronises.  The image upload runs on a second stream
+ * underneath slicing.  slices_out [host] may be NULL; if not, the fp32 intensity slices
+ * [M][P] are downloaded too.  Device buffers are cached inside ctx between calls.
+ */
+SPF_API int spf_orientation_match_host(spf_ctx *ctx, const float *model, const float *quats, int64_t M,
+                                       const float *pix_q, int64_t P, float scale, const float *images,
+                                       int64_t n_img, const uint8_t *mask, int32_t *best_idx, float *best_dist,
+                                       float *slices_out);
+
+/*
+ * Inspection for tests (steps a1-a2 parity): copies the deapodisation factors (n doubles,
+ * index i <-> n = i - floor(N/2)) to a [host] array, and the fine grid in natural FFT order
+ * ([n_fine]^3 complex64, index l mod n_fine) to a [dev] array.  The latter synchronises.
+ */
+SPF_API int spf_debug_deapodisation(const spf_ctx *ctx, double *out_host);
+SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stream);
+
+/*
+ * Test/benchmark knobs (defaults in brackets):
+ *   "slice_impl":  [0] shared-memory-staged gather (TMA tile loads); 1 = plain global-memory gather
+ *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
+ *   "match_cta_group": [2] CTAs per tcgen05 MMA (2 = cta_group::2 pairs, 1 = single CTA)
+ * Returns SPF_EINVAL for an unknown key or value.
+ */
+SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
+
+/*
+ * Device-time statistics of the last spf_slice / spf_match, for bench.py: counts of launches
+ * this library made since the context was created (so the harness can report gpu_launches).
+ */
+SPF_API int64_t spf_launch_count(const spf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPF_H_ */

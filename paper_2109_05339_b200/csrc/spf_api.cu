@@ -1,0 +1,160 @@
+// libspf: context life cycle, errors, options, and the host-buffer entry point.
+#include <math.h>
+#include <stdarg.h>
+
+#include "spf_internal.cuh"
+
+static std::string g_create_err;
+
+int spf_set_err(spf_ctx *ctx, int code, const char *fmt, ...) {
+    char buf[1024];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf;
+    else g_create_err = buf;
+    return code;
+}
+
+// ------------------------------------------------------------------------------------------
+// host-buffer entry point
+// ------------------------------------------------------------------------------------------
+template <typename T>
+static int grow(spf_ctx *ctx, T **p, size_t *cap, size_t bytes) {
+    if (bytes <= *cap && *p) return SPF_OK;
+    if (*p) { cudaFree(*p); *p = nullptr; *cap = 0; }
+    if (bytes == 0) bytes = 16;
+    SPF_CUDA(ctx, cudaMalloc((void **)p, bytes));
+    *cap = bytes;
+    return SPF_OK;
+}
+
+extern "C" {
+
+const char *spf_version(void) { return "libspf 0.1 (sm_100a)"; }
+
+const char *spf_status_string(int s) {
+    switch (s) {
+        case SPF_OK: return "SPF_OK";
+        case SPF_EINVAL: return "SPF_EINVAL";
+        case SPF_ENOMEM: return "SPF_ENOMEM";
+        case SPF_ECUDA: return "SPF_ECUDA";
+        case SPF_ESTATE: return "SPF_ESTATE";
+        default: return "SPF_UNKNOWN";
+    }
+}
+
+const char *spf_last_error(const spf_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+// w = ceil(log10(1/eps)) + 1 (reading s10), clamped to [2, SPF_MAX_W]
+int32_t spf_plan_kernel_width(double eps) {
+    if (!(eps > 0.0) || eps > 0.1) return -1;
+    int w = (int)ceil(log10(1.0 / eps) - 1e-9) + 1;
+    if (w < 2) w = 2;
+    if (w > SPF_MAX_W) w = SPF_MAX_W;
+    return w;
+}
+
+static bool smooth2357(int v) {
+    for (int p : {2, 3, 5, 7})
+        while (v % p == 0) v /= p;
+    return v == 1;
+}
+
+// smallest even 2-3-5-7-smooth integer >= upsampfac * n: cuFFT then needs no Bluestein pass
+// (2 * 151 = 302 has the prime factor 151; the next smooth even size is 320)
+int32_t spf_plan_n_fine(int32_t n, double upsampfac) {
+    if (n < 2 || !(upsampfac >= 2.0)) return -1;
+    int v = (int)ceil(upsampfac * n - 1e-9);
+    if (v % 2) ++v;
+    while (!smooth2357(v)) v += 2;
+    return v;
+}
+
+int spf_get_info(const spf_ctx *ctx, spf_info *out) {
+    if (!ctx || !out) return SPF_EINVAL;
+    out->n = ctx->n; out->n_fine = ctx->nf; out->w = ctx->w; out->beta = ctx->beta;
+    out->n_padded = ctx->np; out->grid_is_real = ctx->grid_is_real ? 1 : 0;
+    out->prepared = ctx->prepared ? 1 : 0; out->sm_count = ctx->sm_count;
+    return SPF_OK;
+}
+
+int spf_set_detector_layout(spf_ctx *ctx, int32_t n_panels, int32_t rows, int32_t cols) {
+    if (!ctx) return SPF_EINVAL;
+    if (n_panels == 0) { ctx->lay_panels = ctx->lay_rows = ctx->lay_cols = 0; return SPF_OK; }
+    if (n_panels < 0 || rows <= 0 || cols <= 0) return spf_set_err(ctx, SPF_EINVAL, "detector layout sizes must be positive");
+    ctx->lay_panels = n_panels; ctx->lay_rows = rows; ctx->lay_cols = cols;
+    return SPF_OK;
+}
+
+int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
+    if (!ctx || !key) return SPF_EINVAL;
+    if (!strcmp(key, "slice_impl") && (value == 0 || value == 1)) { ctx->opt_slice_impl = (int)value; return SPF_OK; }
+    if (!strcmp(key, "force_complex_grid") && (value == 0 || value == 1)) { ctx->opt_force_complex = (int)value; return SPF_OK; }
+    if (!strcmp(key, "match_cta_group") && (value == 1 || value == 2)) { ctx->opt_match_cta_group = (int)value; return SPF_OK; }
+    return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
+}
+
+int64_t spf_launch_count(const spf_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int spf_orientation_match_host(spf_ctx *ctx, const float *model, const float *quats, int64_t M, const float *pix_q,
+                               int64_t P, float scale, const float *images, int64_t n_img, const uint8_t *mask,
+                               int32_t *best_idx, float *best_dist, float *slices_out) {
+    if (!ctx) return SPF_EINVAL;
+    if (!model || !quats || !pix_q || !images || !best_idx || !best_dist || M < 1 || P < 1 || n_img < 1)
+        return spf_set_err(ctx, SPF_EINVAL, "spf_orientation_match_host: null pointer or non-positive size");
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    auto &b = ctx->hb;
+    if (!b.s_main) {
+        SPF_CUDA(ctx, cudaStreamCreateWithFlags(&b.s_main, cudaStreamNonBlocking));
+        SPF_CUDA(ctx, cudaStreamCreateWithFlags(&b.s_copy, cudaStreamNonBlocking));
+        SPF_CUDA(ctx, cudaEventCreateWithFlags(&b.ev_img, cudaEventDisableTiming));
+    }
+    const size_t n3 = (size_t)ctx->n * ctx->n * ctx->n;
+    const size_t ws_bytes = spf_match_workspace_bytes(n_img, M, P);
+    int rc;
+    if ((rc = grow(ctx, &b.model, &b.cap_model, n3 * 4))) return rc;
+    if ((rc = grow(ctx, &b.quats, &b.cap_quats, (size_t)M * 16))) return rc;
+    if ((rc = grow(ctx, &b.pix, &b.cap_pix, (size_t)P * 12))) return rc;
+    if ((rc = grow(ctx, &b.images, &b.cap_images, (size_t)n_img * P * 4))) return rc;
+    if ((rc = grow(ctx, &b.slices, &b.cap_slices, (size_t)M * P * 4))) return rc;
+    if ((rc = grow(ctx, &b.mask, &b.cap_mask, (size_t)P))) return rc;
+    if ((rc = grow(ctx, &b.bidx, &b.cap_bi, (size_t)n_img * 4))) return rc;
+    if ((rc = grow(ctx, &b.bdist, &b.cap_bd, (size_t)n_img * 4))) return rc;
+    if ((rc = grow(ctx, &b.ws, &b.cap_ws, ws_bytes))) return rc;
+
+    // images (the large input) upload on the copy stream, underneath prepare + slice
+    SPF_CUDA(ctx, cudaMemcpyAsync(b.images, images, (size_t)n_img * P * 4, cudaMemcpyHostToDevice, b.s_copy));
+    SPF_CUDA(ctx, cudaEventRecord(b.ev_img, b.s_copy));
+    SPF_CUDA(ctx, cudaMemcpyAsync(b.model, model, n3 * 4, cudaMemcpyHostToDevice, b.s_main));
+    SPF_CUDA(ctx, cudaMemcpyAsync(b.quats, quats, (size_t)M * 16, cudaMemcpyHostToDevice, b.s_main));
+    SPF_CUDA(ctx, cudaMemcpyAsync(b.pix, pix_q, (size_t)P * 12, cudaMemcpyHostToDevice, b.s_main));
+    if (mask) SPF_CUDA(ctx, cudaMemcpyAsync(b.mask, mask, (size_t)P, cudaMemcpyHostToDevice, b.s_main));
+    if ((rc = spf_prepare_model(ctx, b.model, b.s_main))) return rc;
+    if ((rc = spf_slice(ctx, b.quats, M, b.pix, P, SPF_OUT_INTENSITY, scale, b.slices, b.s_main))) return rc;
+    SPF_CUDA(ctx, cudaStreamWaitEvent(b.s_main, b.ev_img, 0));
+    if ((rc = spf_match(ctx, b.images, n_img, b.slices, M, P, mask ? b.mask : nullptr, b.bidx, b.bdist, b.ws, ws_bytes,
+                        b.s_main)))
+        return rc;
+    SPF_CUDA(ctx, cudaMemcpyAsync(best_idx, b.bidx, (size_t)n_img * 4, cudaMemcpyDeviceToHost, b.s_main));
+    SPF_CUDA(ctx, cudaMemcpyAsync(best_dist, b.bdist, (size_t)n_img * 4, cudaMemcpyDeviceToHost, b.s_main));
+    if (slices_out)
+        SPF_CUDA(ctx, cudaMemcpyAsync(slices_out, b.slices, (size_t)M * P * 4, cudaMemcpyDeviceToHost, b.s_main));
+    SPF_CUDA(ctx, cudaStreamSynchronize(b.s_main));
+    return SPF_OK;
+}
+
+}  // extern "C"
+
+spf_encode_tiled_fn spf_get_encode_tiled() {
+    static spf_encode_tiled_fn fn = nullptr;
+    if (fn) return fn;
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+        return nullptr;
+    fn = (spf_encode_tiled_fn)p;
+    return fn;
+}

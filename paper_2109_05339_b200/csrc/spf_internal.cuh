@@ -1,0 +1,105 @@
+// Internal declarations of libspf (not part of the ABI).  sm_100a only.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/spf.h"
+
+#define SPF_MAX_W 16
+
+// One TMA tensor map per (box_z, box_y) combination used by the slicing kernel to stage a
+// fine-grid tile: boxes are {SPF_BOX_MIN, +4, ..., SPF_BOX_MAX} cells along z and y, one x-plane deep.
+#define SPF_BOX_MIN 8
+#define SPF_BOX_MAX 40
+#define SPF_BOX_STEP 4
+#define SPF_BOX_N ((SPF_BOX_MAX - SPF_BOX_MIN) / SPF_BOX_STEP + 1)  // 9
+
+struct SliceMaps {
+    CUtensorMap m[SPF_BOX_N * SPF_BOX_N];  // [iy * SPF_BOX_N + iz]
+};
+
+struct spf_ctx {
+    spf_params prm{};
+    int n = 0, nf = 0, w = 0, halo = 0, np = 0;  // np: padded edge (x and y); sz: z pitch (>= np, multiple of 4)
+    int sz = 0;
+    double beta = 0.0;
+    int sm_count = 0;
+    bool prepared = false;
+    bool grid_is_real = false;
+    int opt_slice_impl = 0;
+    int opt_force_complex = 0;
+    int opt_match_cta_group = 2;
+    int64_t launches = 0;
+
+    std::vector<double> deapod;  // host, n entries
+    float *d_deapod = nullptr;   // device fp32 copy (n)
+    float2 *d_fft = nullptr;     // n_fine^3 complex, natural order (FFT in place)
+    float2 *d_gridc = nullptr;   // np*np*sz complex, centred + halo
+    float *d_gridr = nullptr;    // np*np*sz real, centred + halo (valid when grid_is_real)
+    int *d_flag = nullptr;       // 1 int: model-not-even counter
+    cufftHandle plan = 0;
+    bool plan_ok = false;
+    void *d_fft_work = nullptr;
+    size_t fft_work_bytes = 0;
+
+    // detector layout promise
+    int lay_panels = 0, lay_rows = 0, lay_cols = 0;
+    int32_t *d_patch = nullptr;  // [n_patches][SPF_PATCH] pixel indices, -1 = empty
+    int64_t patch_P = -1;        // P the patch table was built for
+    int patch_key[3] = {-1, -1, -1};
+    int64_t n_patches = 0;
+
+    SliceMaps maps_c{}, maps_r{};
+    bool maps_ok = false;
+
+    // host-buffer entry point: cached device buffers
+    struct HostBufs {
+        float *model = nullptr, *quats = nullptr, *pix = nullptr, *images = nullptr, *slices = nullptr, *bdist = nullptr;
+        uint8_t *mask = nullptr;
+        int32_t *bidx = nullptr;
+        void *ws = nullptr;
+        size_t cap_model = 0, cap_quats = 0, cap_pix = 0, cap_images = 0, cap_slices = 0, cap_mask = 0, cap_bi = 0, cap_bd = 0, cap_ws = 0;
+        cudaStream_t s_main = nullptr, s_copy = nullptr;
+        cudaEvent_t ev_img = nullptr;
+    } hb;
+
+    std::string err;
+};
+
+#define SPF_PATCH 128  // threads per slicing block = pixels per patch
+
+int spf_set_err(spf_ctx *ctx, int code, const char *fmt, ...);
+
+#define SPF_CUDA(ctx, call)                                                                      \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess)                                                                   \
+            return spf_set_err((ctx), e_ == cudaErrorMemoryAllocation ? SPF_ENOMEM : SPF_ECUDA, \
+                               "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+#define SPF_LAUNCH_CHECK(ctx)                                                                                   \
+    do {                                                                                                        \
+        cudaError_t e_ = cudaGetLastError();                                                                    \
+        if (e_ != cudaSuccess)                                                                                  \
+            return spf_set_err((ctx), SPF_ECUDA, "kernel launch failed: %s (%s:%d)", cudaGetErrorString(e_), __FILE__, \
+                               __LINE__);                                                                       \
+        (ctx)->launches++;                                                                                      \
+    } while (0)
+
+// driver entry point for cuTensorMapEncodeTiled fetched through the runtime (no -lcuda needed)
+typedef CUresult (*spf_encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                        const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                        CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                        CUtensorMapFloatOOBfill);
+spf_encode_tiled_fn spf_get_encode_tiled();
+
+// implemented in spf_prepare.cu / spf_slice.cu / spf_match.cu
+int spf_build_slice_maps(spf_ctx *ctx);

@@ -1,0 +1,476 @@
+// libspf: spf_match (steps a6-a8 of SURVEY.md section 8(a)).
+//
+//   d[i][m] = ||I_i||^2 + ||S_m||^2 - 2 I_i . S_m   over unmasked pixels,  best_i = argmin_m d[i][m]
+//
+// The cross term is a dense contraction (n_img x P) . (M x P)^T and runs on the 5th-generation tensor
+// cores: tcgen05.mma with fp32 accumulators in TMEM, operands staged in shared memory by TMA.
+// fp32-equivalent products come from a two-term fp16 split of each operand, x * 2^e = h1 + h2 (+ <=2^-22
+// relative), after a power-of-two rescale into fp16 range.  Photon-count images are exact in ONE fp16
+// term (integers < 2048), which is tested on the device: the kernel instantiated for one image plane
+// issues 2 products per K step (I1.S1, I1.S2), the one for two planes issues 3 (adds I2.S1).  Both
+// instantiations are launched and the one the data does not need returns at once, so the host never
+// synchronises.  The epilogue reads the accumulator tile out of TMEM, adds the norms and keeps a
+// running (min, argmin) per image row; tiles merge through a 64-bit atomicMin on
+// (order-preserving bits of d) << 32 | m, so the lowest index wins exact ties and the distance
+// matrix never exists in memory.
+#include <cuda_fp16.h>
+#include <math.h>
+
+#include "ptx_sm100.cuh"
+#include "spf_internal.cuh"
+
+namespace {
+
+constexpr int BK = 64;                            // fp16 elements per K block: 128 bytes, one swizzle row
+constexpr int BN = 256;                           // slices per tile (UMMA N)
+constexpr int TILE_ROWS = 128;                    // image rows per CTA (UMMA M = 128 * CG)
+constexpr int A_TILE_BYTES = TILE_ROWS * BK * 2;  // 16 KB
+constexpr int GEMM_THREADS = 192;                 // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
+constexpr int ACC_STAGES = 2;
+constexpr int TMEM_COLS = ACC_STAGES * BN;        // 512: all of TMEM, one CTA per SM
+constexpr size_t SMEM_AUX = 4096;                 // barriers, tmem pointer, ||S||^2 tile buffers
+constexpr size_t SMEM_BUDGET = 227 * 1024;
+
+template <int CG, int NI>
+struct GemmCfg {
+    static constexpr int B_ROWS = BN / CG;                      // slice rows this CTA stages
+    static constexpr int B_TILE_BYTES = B_ROWS * BK * 2;
+    static constexpr int STAGE_BYTES = NI * A_TILE_BYTES + 2 * B_TILE_BYTES;
+    static constexpr int STAGES_RAW = (int)((SMEM_BUDGET - SMEM_AUX - 1024) / STAGE_BYTES);
+    static constexpr int STAGES = STAGES_RAW > 6 ? 6 : STAGES_RAW;
+    static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + SMEM_AUX + 1024;
+    static_assert(STAGES >= 2, "need at least a double buffer");
+};
+
+struct MatchArgs {
+    int64_t n_img, M;
+    int kblocks;            // P_pad / 64
+    int n_ib, n_mb;         // tiles along images / slices
+    unsigned long long *keys;
+    const float *nI, *nS;
+    const uint32_t *scal;   // [2] = image plane 2 needed, [4] = eI, [5] = eS
+};
+
+struct WsLayout {
+    size_t scal, keys, nI, nS, planesI, planesS, total;
+    int64_t Ppad;
+};
+
+size_t rup(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+WsLayout ws_layout(int64_t n_img, int64_t M, int64_t P) {
+    WsLayout L{};
+    L.Ppad = (int64_t)rup((size_t)P, BK);
+    size_t off = 0;
+    L.scal = off; off += 1024;
+    L.keys = off; off += rup((size_t)n_img * 8, 1024);
+    L.nI = off; off += rup((size_t)n_img * 4, 1024);
+    L.nS = off; off += rup((size_t)M * 4, 1024);
+    L.planesI = off; off += rup((size_t)2 * n_img * L.Ppad * 2, 1024);
+    L.planesS = off; off += rup((size_t)2 * M * L.Ppad * 2, 1024);
+    L.total = off;
+    return L;
+}
+
+// ------------------------------------------------------------------------------------------
+// a6 + operand preparation
+// ------------------------------------------------------------------------------------------
+// max |x| over unmasked pixels, as the bit pattern of a non-negative float (orders like an unsigned)
+__global__ void k_absmax(const float *__restrict__ x, int64_t rows, int64_t P, const uint8_t *__restrict__ mask,
+                         uint32_t *__restrict__ out) {
+    uint32_t m = 0;
+    const int64_t total = rows * P;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        if (mask && !mask[idx % P]) continue;
+        m = max(m, __float_as_uint(fabsf(x[idx])));
+    }
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
+__device__ __forceinline__ int scale_exponent(uint32_t absmax_bits) {
+    // 2^e * max in [2^14, 2^15): fp16 holds it with 11 significant bits, products stay far from overflow
+    float mx = __uint_as_float(absmax_bits);
+    if (!(mx > 0.0f) || isinf(mx) || isnan(mx)) return 0;
+    int k;
+    frexpf(mx, &k);  // mx = f * 2^k, f in [0.5, 1)
+    int e = 15 - k;
+    return max(-100, min(100, e));
+}
+
+// One block per row: x * 2^e = h1 + h2 as two fp16 planes (zero in masked pixels and in the K padding),
+// ||x||^2 over unmasked pixels accumulated in fp64, and (images) the running-argmin key reset.
+// which = 0: images (sets scal[2] when some residual is non-zero, resets keys), 1: slices.
+__global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int64_t P, int64_t Ppad,
+                                               const uint8_t *__restrict__ mask, uint32_t *__restrict__ scal, int which,
+                                               int64_t rows, __half *__restrict__ planes, float *__restrict__ norms,
+                                               unsigned long long *__restrict__ keys) {
+    const int64_t row = blockIdx.x;
+    const int e = scale_exponent(scal[which]);
+    const float sc = ldexpf(1.0f, e);
+    const float *xr = x + row * P;
+    __half *h1 = planes + row * Ppad, *h2 = planes + (rows + row) * Ppad;
+    double acc = 0.0;
+    bool inexact = false;
+    for (int64_t c = threadIdx.x; c < Ppad; c += blockDim.x) {
+        float v = 0.0f;
+        if (c < P && (!mask || mask[c])) v = xr[c];
+        acc += (double)v * (double)v;
+        float vs = v * sc;
+        __half a = __float2half_rn(vs);
+        float r = vs - __half2float(a);
+        __half b = __float2half_rn(r);
+        inexact |= (r != 0.0f);
+        h1[c] = a;
+        h2[c] = b;
+    }
+    __shared__ double red[8];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    const bool any = __any_sync(0xffffffffu, inexact);
+    if ((threadIdx.x & 31) == 0) {
+        red[threadIdx.x >> 5] = acc;
+        if (which == 0 && any) atomicOr(&scal[2], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) s += red[k];
+        norms[row] = (float)s;
+        if (which == 0) keys[row] = ~0ull;
+        if (row == 0) scal[4 + which] = (uint32_t)e;
+    }
+}
+
+__device__ __forceinline__ uint32_t orderable(float d) {
+    uint32_t u = __float_as_uint(d);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float unorderable(uint32_t u) {
+    return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
+}
+
+__global__ void k_match_finalize(const unsigned long long *__restrict__ keys, int64_t n_img, int32_t *__restrict__ best_idx,
+                                 float *__restrict__ best_dist) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n_img) return;
+    unsigned long long k = keys[i];
+    best_idx[i] = (int32_t)(uint32_t)(k & 0xffffffffull);  // -1 if no finite distance was seen
+    best_dist[i] = (k == ~0ull) ? __uint_as_float(0x7fc00000u) : unorderable((uint32_t)(k >> 32));
+}
+
+// ------------------------------------------------------------------------------------------
+// a7 + a8: tcgen05 GEMM with the fused norm-add / argmin epilogue
+// ------------------------------------------------------------------------------------------
+template <int CG, int NI>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
+             const __grid_constant__ CUtensorMap mapB0, const __grid_constant__ CUtensorMap mapB1, const MatchArgs a) {
+    using Cfg = GemmCfg<CG, NI>;
+    constexpr int ST = Cfg::STAGES;
+    // the instantiation the data does not need leaves before touching any barrier or TMEM
+    if ((a.scal[2] != 0u) != (NI == 2)) return;
+
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;  // SWIZZLE_128B tiles need 1024-byte alignment
+    uint8_t *smem_al = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
+    const uint32_t aux = smem_base + ST * Cfg::STAGE_BYTES;
+    uint8_t *aux_p = smem_al + (size_t)ST * Cfg::STAGE_BYTES;
+    const uint32_t bar_full = aux, bar_empty = aux + 8 * ST, bar_tfull = aux + 16 * ST, bar_tempty = bar_tfull + 8 * ACC_STAGES;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(aux_p + 16 * ST + 16 * ACC_STAGES);
+    float *nsbuf = reinterpret_cast<float *>(aux_p + 1024);  // [ACC_STAGES][BN]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
+    const bool leader = (rank == 0);
+    const int cluster_id = blockIdx.x / CG, n_clusters = gridDim.x / CG;
+    const int n_tiles = a.n_ib * a.n_mb;
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&mapA0); ptx::prefetch_tensormap(&mapB0); ptx::prefetch_tensormap(&mapB1);
+        if (NI == 2) ptx::prefetch_tensormap(&mapA1);
+        for (int s = 0; s < ST; ++s) { ptx::mbar_init(bar_full + 8 * s, 1); ptx::mbar_init(bar_empty + 8 * s, 1); }
+        for (int s = 0; s < ACC_STAGES; ++s) { ptx::mbar_init(bar_tfull + 8 * s, 1); ptx::mbar_init(bar_tempty + 8 * s, 4 * CG); }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) ptx::tmem_alloc<CG>(ptx::smem_u32(tmem_slot), TMEM_COLS);
+    ptx::tc_fence_before();
+    if (CG == 2) ptx::cluster_sync(); else __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    auto tile_coords = [&](int t, int &ib, int &mb) {
+        // groups of 8 image blocks, slice tiles fastest across groups' members: concurrently
+        // running tiles share operand rows in L2
+        const int G = 8;
+        const int per_group = G * a.n_mb;
+        const int g = t / per_group, r = t - g * per_group;
+        const int gsz = min(G, a.n_ib - g * G);
+        ib = g * G + r % gsz;
+        mb = r / gsz;
+    };
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        int s = 0; uint32_t ph = 0;
+        for (int t = cluster_id; t < n_tiles; t += n_clusters) {
+            int ib, mb; tile_coords(t, ib, mb);
+            const int rowA = ib * (TILE_ROWS * CG) + (int)rank * TILE_ROWS;
+            const int rowB = mb * BN + (int)rank * Cfg::B_ROWS;
+            for (int kb = 0; kb < a.kblocks; ++kb) {
+                ptx::mbar_wait(bar_empty + 8 * s, ph ^ 1u);
+                if (lane == 0) {
+                    const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
+                    const uint32_t fb = bar_full + 8 * s;
+                    if (CG == 1) ptx::mbar_expect_tx(fb, Cfg::STAGE_BYTES);
+                    else if (leader) ptx::mbar_expect_tx(fb, 2 * Cfg::STAGE_BYTES);
+                    const int kc = kb * BK;
+                    if (CG == 1) {
+                        ptx::tma_load_2d(st, &mapA0, kc, rowA, fb);
+                        if (NI == 2) ptx::tma_load_2d(st + A_TILE_BYTES, &mapA1, kc, rowA, fb);
+                        ptx::tma_load_2d(st + NI * A_TILE_BYTES, &mapB0, kc, rowB, fb);
+                        ptx::tma_load_2d(st + NI * A_TILE_BYTES + Cfg::B_TILE_BYTES, &mapB1, kc, rowB, fb);
+                    } else {
+                        ptx::tma_load_2d_2sm(st, &mapA0, kc, rowA, fb);
+                        if (NI == 2) ptx::tma_load_2d_2sm(st + A_TILE_BYTES, &mapA1, kc, rowA, fb);
+                        ptx::tma_load_2d_2sm(st + NI * A_TILE_BYTES, &mapB0, kc, rowB, fb);
+                        ptx::tma_load_2d_2sm(st + NI * A_TILE_BYTES + Cfg::B_TILE_BYTES, &mapB1, kc, rowB, fb);
+                    }
+                }
+                __syncwarp();
+                if (++s == ST) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (leader CTA of the pair) =====================
+        if (leader) {
+            constexpr uint32_t idesc = ptx::umma_idesc_f16(TILE_ROWS * CG, BN);
+            int s = 0; uint32_t ph = 0; int as = 0; uint32_t aph = 0;
+            for (int t = cluster_id; t < n_tiles; t += n_clusters) {
+                ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u);  // epilogue has drained this accumulator stage
+                ptx::tc_fence_after();
+                const uint32_t tacc = tmem_base + (uint32_t)(as * BN);
+                for (int kb = 0; kb < a.kblocks; ++kb) {
+                    ptx::mbar_wait(bar_full + 8 * s, ph);
+                    ptx::tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
+                        const uint64_t dA0 = ptx::umma_desc_sw128(st);
+                        const uint64_t dA1 = ptx::umma_desc_sw128(st + A_TILE_BYTES);
+                        const uint64_t dB0 = ptx::umma_desc_sw128(st + NI * A_TILE_BYTES);
+                        const uint64_t dB1 = ptx::umma_desc_sw128(st + NI * A_TILE_BYTES + Cfg::B_TILE_BYTES);
+#pragma unroll
+                        for (int k4 = 0; k4 < BK / 16; ++k4) {  // 16 fp16 = 32 bytes per UMMA K step: +2 in the address field
+                            const uint64_t ko = (uint64_t)(k4 * 2);
+                            ptx::umma_f16<CG>(tacc, dA0 + ko, dB0 + ko, idesc, (uint32_t)((kb | k4) != 0));
+                            ptx::umma_f16<CG>(tacc, dA0 + ko, dB1 + ko, idesc, 1u);
+                            if (NI == 2) ptx::umma_f16<CG>(tacc, dA1 + ko, dB0 + ko, idesc, 1u);
+                        }
+                        ptx::umma_commit<CG>(bar_empty + 8 * s);                              // smem slot free when these MMAs retire
+                        if (kb == a.kblocks - 1) ptx::umma_commit<CG>(bar_tfull + 8 * as);   // accumulator complete
+                    }
+                    __syncwarp();
+                    if (++s == ST) { s = 0; ph ^= 1u; }
+                }
+                if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== epilogue: TMEM -> registers -> norm add + running argmin =====================
+        const int q = warp & 3;                 // TMEM lane quadrant this warp may read
+        const int e = (warp - 2) * 32 + lane;   // 0..127 among the epilogue threads
+        const float neg2sc = ldexpf(-2.0f, -((int)a.scal[4] + (int)a.scal[5]));
+        int as = 0; uint32_t aph = 0;
+        for (int t = cluster_id; t < n_tiles; t += n_clusters) {
+            int ib, mb; tile_coords(t, ib, mb);
+            const int64_t m0 = (int64_t)mb * BN;
+            float *nsb = nsbuf + as * BN;
+            for (int k = e; k < BN; k += 128) nsb[k] = (m0 + k < a.M) ? a.nS[m0 + k] : INFINITY;
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            const int64_t i = (int64_t)ib * (TILE_ROWS * CG) + (int64_t)rank * TILE_ROWS + q * 32 + lane;
+            const float nIv = (i < a.n_img) ? a.nI[i] : 0.0f;
+            ptx::mbar_wait(bar_tfull + 8 * as, aph);
+            ptx::tc_fence_after();
+            float best = INFINITY; uint32_t bm = 0xffffffffu;
+            const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * BN);
+#pragma unroll 1
+            for (int c = 0; c < BN / 32; ++c) {
+                uint32_t r[32];
+                ptx::tmem_ld_32x32(trow + c * 32, r);
+                ptx::tmem_ld_wait();
+#pragma unroll
+                for (int k = 0; k < 32; ++k) {
+                    const float d = nIv + fmaf(neg2sc, __uint_as_float(r[k]), nsb[c * 32 + k]);
+                    if (d < best) { best = d; bm = (uint32_t)(m0 + c * 32 + k); }
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) { if (CG == 2) ptx::mbar_arrive_cluster(bar_tempty + 8 * as, 0); else ptx::mbar_arrive(bar_tempty + 8 * as); }
+            if (i < a.n_img && bm != 0xffffffffu)
+                atomicMin(&a.keys[i], ((unsigned long long)orderable(best) << 32) | bm);
+            if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
+        }
+    }
+
+    ptx::tc_fence_before();
+    if (CG == 2) ptx::cluster_sync(); else __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+}
+
+// ------------------------------------------------------------------------------------------
+// reference matcher (tests only): difference form on the CUDA cores, fp64 accumulation
+// ------------------------------------------------------------------------------------------
+__global__ void k_match_ref_dist(const float *__restrict__ images, int64_t n_img, const float *__restrict__ slices, int64_t M,
+                                 int64_t P, const uint8_t *__restrict__ mask, float *__restrict__ dist) {
+    const int64_t pair = blockIdx.x;  // one block per (i, m)
+    const int64_t i = pair / M, m = pair % M;
+    const float *I = images + i * P, *S = slices + m * P;
+    double acc = 0.0;
+    for (int64_t j = threadIdx.x; j < P; j += blockDim.x) {
+        if (mask && !mask[j]) continue;
+        double t = (double)I[j] - (double)S[j];
+        acc += t * t;
+    }
+    __shared__ double red[8];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) s += red[k];
+        dist[pair] = (float)s;
+    }
+}
+
+__global__ void k_match_ref_argmin(const float *__restrict__ dist, int64_t n_img, int64_t M, int32_t *__restrict__ best_idx,
+                                   float *__restrict__ best_dist) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n_img) return;
+    const float *d = dist + i * M;
+    int64_t b = 0;
+    for (int64_t m = 1; m < M; ++m)
+        if (d[m] < d[b]) b = m;
+    best_idx[i] = (int32_t)b;
+    best_dist[i] = d[b];
+}
+
+int encode_operand_map(spf_ctx *ctx, CUtensorMap *map, const void *base, int64_t rows, int64_t Ppad, int box_rows) {
+    spf_encode_tiled_fn enc = spf_get_encode_tiled();
+    if (!enc) return spf_set_err(ctx, SPF_ECUDA, "cuTensorMapEncodeTiled entry point not available");
+    cuuint64_t gdim[2] = {(cuuint64_t)Ppad, (cuuint64_t)rows};
+    cuuint64_t gstr[1] = {(cuuint64_t)Ppad * 2};
+    cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void *>(base), gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return spf_set_err(ctx, SPF_ECUDA, "cuTensorMapEncodeTiled(match operand) failed: %d", (int)r);
+    return SPF_OK;
+}
+
+template <int CG, int NI>
+int launch_gemm(spf_ctx *ctx, const CUtensorMap &a0, const CUtensorMap &a1, const CUtensorMap &b0, const CUtensorMap &b1,
+                const MatchArgs &args, cudaStream_t st) {
+    using Cfg = GemmCfg<CG, NI>;
+    auto kern = k_match_gemm<CG, NI>;
+    SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+    const int n_tiles = args.n_ib * args.n_mb;
+    int clusters = ctx->sm_count / CG;
+    if (clusters > n_tiles) clusters = n_tiles;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(clusters * CG));
+    cfg.blockDim = dim3(GEMM_THREADS);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    SPF_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, a0, a1, b0, b1, args));
+    ctx->launches++;
+    return SPF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t spf_match_workspace_bytes(int64_t n_img, int64_t M, int64_t P) {
+    if (n_img < 0 || M < 0 || P < 0) return 0;
+    return ws_layout(n_img, M, P).total;
+}
+
+int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P,
+              const uint8_t *mask, int32_t *best_idx, float *best_dist, void *workspace, size_t workspace_bytes,
+              void *stream_) {
+    if (!ctx) return SPF_EINVAL;
+    if (n_img < 0 || M < 0 || P < 0) return spf_set_err(ctx, SPF_EINVAL, "spf_match: negative size");
+    if (n_img == 0) return SPF_OK;
+    if (M < 1 || P < 1) return spf_set_err(ctx, SPF_EINVAL, "spf_match: M and P must be >= 1 when n_img >= 1");
+    if (!images || !slices || !best_idx || !best_dist || !workspace) return spf_set_err(ctx, SPF_EINVAL, "spf_match: null pointer");
+    if (M > 0x7fffffffLL || n_img > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: more than 2^31-1 rows");
+    const WsLayout L = ws_layout(n_img, M, P);
+    if (workspace_bytes < L.total) return spf_set_err(ctx, SPF_EINVAL, "spf_match: workspace %zu < required %zu bytes", workspace_bytes, L.total);
+    if (((uintptr_t)workspace & 1023u) != 0) return spf_set_err(ctx, SPF_EINVAL, "spf_match: workspace must be 1024-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream_;
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    uint8_t *ws = (uint8_t *)workspace;
+    uint32_t *scal = (uint32_t *)(ws + L.scal);
+    unsigned long long *keys = (unsigned long long *)(ws + L.keys);
+    float *nI = (float *)(ws + L.nI), *nS = (float *)(ws + L.nS);
+    __half *plI = (__half *)(ws + L.planesI), *plS = (__half *)(ws + L.planesS);
+
+    SPF_CUDA(ctx, cudaMemsetAsync(scal, 0, 64, st));
+    const int rb = ctx->sm_count * 8;
+    k_absmax<<<rb, 256, 0, st>>>(images, n_img, P, mask, scal + 0);
+    SPF_LAUNCH_CHECK(ctx);
+    k_absmax<<<rb, 256, 0, st>>>(slices, M, P, mask, scal + 1);
+    SPF_LAUNCH_CHECK(ctx);
+    k_split<<<(unsigned)n_img, 256, 0, st>>>(images, P, L.Ppad, mask, scal, 0, n_img, plI, nI, keys);
+    SPF_LAUNCH_CHECK(ctx);
+    k_split<<<(unsigned)M, 256, 0, st>>>(slices, P, L.Ppad, mask, scal, 1, M, plS, nS, nullptr);
+    SPF_LAUNCH_CHECK(ctx);
+
+    const int CG = ctx->opt_match_cta_group;
+    CUtensorMap a0, a1, b0, b1;
+    int rc;
+    if ((rc = encode_operand_map(ctx, &a0, plI, n_img, L.Ppad, TILE_ROWS))) return rc;
+    if ((rc = encode_operand_map(ctx, &a1, plI + (size_t)n_img * L.Ppad, n_img, L.Ppad, TILE_ROWS))) return rc;
+    if ((rc = encode_operand_map(ctx, &b0, plS, M, L.Ppad, BN / CG))) return rc;
+    if ((rc = encode_operand_map(ctx, &b1, plS + (size_t)M * L.Ppad, M, L.Ppad, BN / CG))) return rc;
+    MatchArgs args{};
+    args.n_img = n_img; args.M = M; args.kblocks = (int)(L.Ppad / BK);
+    args.n_ib = (int)((n_img + TILE_ROWS * CG - 1) / (TILE_ROWS * CG));
+    args.n_mb = (int)((M + BN - 1) / BN);
+    args.keys = keys; args.nI = nI; args.nS = nS; args.scal = scal;
+    if ((int64_t)args.n_ib * args.n_mb > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: too many tiles");
+    if (CG == 2) {
+        if ((rc = launch_gemm<2, 1>(ctx, a0, a1, b0, b1, args, st))) return rc;
+        if ((rc = launch_gemm<2, 2>(ctx, a0, a1, b0, b1, args, st))) return rc;
+    } else {
+        if ((rc = launch_gemm<1, 1>(ctx, a0, a1, b0, b1, args, st))) return rc;
+        if ((rc = launch_gemm<1, 2>(ctx, a0, a1, b0, b1, args, st))) return rc;
+    }
+    k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
+    SPF_LAUNCH_CHECK(ctx);
+    return SPF_OK;
+}
+
+int spf_match_reference(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P,
+                        const uint8_t *mask, int32_t *best_idx, float *best_dist, float *dist, void *stream_) {
+    if (!ctx) return SPF_EINVAL;
+    if (n_img < 0 || M < 0 || P < 0) return spf_set_err(ctx, SPF_EINVAL, "spf_match_reference: negative size");
+    if (n_img == 0) return SPF_OK;
+    if (M < 1 || P < 1) return spf_set_err(ctx, SPF_EINVAL, "spf_match_reference: M and P must be >= 1");
+    if (!images || !slices || !best_idx || !best_dist || !dist) return spf_set_err(ctx, SPF_EINVAL, "spf_match_reference: null pointer");
+    if (n_img * M > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match_reference: n_img*M too large (tests only)");
+    cudaStream_t st = (cudaStream_t)stream_;
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    k_match_ref_dist<<<(unsigned)(n_img * M), 256, 0, st>>>(images, n_img, slices, M, P, mask, dist);
+    SPF_LAUNCH_CHECK(ctx);
+    k_match_ref_argmin<<<(unsigned)((n_img + 127) / 128), 128, 0, st>>>(dist, n_img, M, best_idx, best_dist);
+    SPF_LAUNCH_CHECK(ctx);
+    return SPF_OK;
+}
+
+}  // extern "C"

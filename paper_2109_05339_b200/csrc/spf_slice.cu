@@ -1,0 +1,363 @@
+// libspf: spf_slice (steps a3-a5 of SURVEY.md section 8(a)).
+//
+//   c_{m,j} ~= sum_{t1,t2,t3 < w} b[i0 + t] phi1[t1] phi2[t2] phi3[t3],   x = R(quat_m) q_j,  xi = x n_f / 2 pi,
+//   i0 = ceil(xi - w/2),  phi_d[t] = phi(2 (i0_d + t - xi_d) / w),  phi(z) = exp(beta (sqrt(1 - z^2) - 1))
+//
+// One thread block = one orientation x one compact patch of SPF_PATCH detector pixels (an 8 x 16
+// lattice tile when the caller promised a panel layout).  The rotated patch is a small tilted
+// piece of a plane in the fine grid, so its axis-aligned bounding box is a small regular 3-D
+// tile: the block finds the box with a min/max reduction, one warp issues one TMA tensor copy per
+// x-plane of the box into shared memory, and while those are in flight every thread evaluates
+// its 3 w kernel weights (piecewise polynomials, Horner).  The gather then reads shared memory
+// only.  The stored grid is centred with a periodic halo (spf_prepare_model), so there is no
+// modulo anywhere, and it is real fp32 when the model is even -- half the bytes per neighbour.
+// Coordinates (rotation, scaling to cells, split into integer cell + fraction) are fp64: an fp32
+// error of one ulp at |xi| ~ 150 cells is 1.5e-5 cells, which a model that fills the grid turns
+// into a 1e-5 relative error, the whole parity budget.
+#include <limits.h>
+#include <math.h>
+
+#include <vector>
+
+#include "ptx_sm100.cuh"
+#include "spf_internal.cuh"
+
+#define SPF_MAX_DEG 12
+
+namespace {
+
+struct SliceArgs {
+    const float *quats, *pix_q;
+    const int32_t *patch;   // [n_patches][SPF_PATCH]
+    int64_t M, P, n_patches;
+    void *out;
+    float scale;
+    const float *grid;      // centred padded grid, fp32 (REAL) or interleaved complex
+    int np, sz, off, nf, w, deg;
+    double xi_scale;        // n_f / (2 pi)
+    double inv_nf;
+    float beta;
+    uint32_t cap_bytes;     // dynamic shared memory available for the tile
+    float coef[SPF_MAX_W][SPF_MAX_DEG + 1];  // phi at tap t as a polynomial in u = 2 (f + w/2) - 1
+    SliceMaps maps;
+};
+
+// rotation matrix of the normalised quaternion, fp64 (reading s2: Hamilton, active)
+__device__ void quat_to_R(const float *q4, double *R) {
+    double w = q4[0], x = q4[1], y = q4[2], z = q4[3];
+    const double inv = 1.0 / sqrt(w * w + x * x + y * y + z * z);
+    w *= inv; x *= inv; y *= inv; z *= inv;
+    R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
+    R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
+    R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
+}
+
+// one axis: rotated coordinate (radians) -> first padded cell index and fraction f = i0 - xi in [-w/2, -w/2 + 1)
+__device__ __forceinline__ void cell_and_fraction(double x, const SliceArgs &a, int w, int &p, float &f) {
+    double xi = x * a.xi_scale;
+    xi -= (double)a.nf * rint(xi * a.inv_nf);  // 2 pi-periodic: fold into [-n_f/2, n_f/2]
+    const double c = ceil(xi - 0.5 * (double)w);
+    p = (int)c + a.off;
+    f = (float)(c - xi);
+}
+
+// weights by the definition (slice_impl = 1): exp(beta (sqrt(1-z^2) - 1)) written as exp(-beta z^2 / (1 + sqrt(1-z^2)))
+template <int WMAX>
+__device__ __forceinline__ void weights_direct(float f, int w, float beta, float (&wt)[WMAX]) {
+    const float s2w = 2.0f / (float)w;
+#pragma unroll
+    for (int t = 0; t < WMAX; ++t) {
+        if (t < w) {
+            const float z = (f + (float)t) * s2w;
+            const float om = fmaxf(fmaf(-z, z, 1.0f), 0.0f);
+            wt[t] = expf(-beta * z * z / (1.0f + sqrtf(om)));
+        }
+    }
+}
+
+// weights by per-tap polynomials in u (Horner, FMA pipe only)
+template <int WMAX>
+__device__ __forceinline__ void weights_poly(float f, int w, const SliceArgs &a, float (&wt)[WMAX]) {
+    const float u = fmaf(2.0f, f, (float)w - 1.0f);  // 2 (f + w/2) - 1
+#pragma unroll
+    for (int t = 0; t < WMAX; ++t) {
+        if (t < w) {
+            float p = a.coef[t][a.deg];
+            for (int k = a.deg - 1; k >= 0; --k) p = fmaf(p, u, a.coef[t][k]);
+            wt[t] = p;
+        }
+    }
+}
+
+// sum over the w^3 neighbours; `base` points at cell (i0x, i0y, i0z), strides in cells
+template <int WMAX, bool REAL>
+__device__ __forceinline__ float2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMAX],
+                                         const float (&wy)[WMAX], const float (&wz)[WMAX]) {
+    float accr = 0.0f, acci = 0.0f;
+    constexpr int E = REAL ? 1 : 2;
+#pragma unroll 1
+    for (int t1 = 0; t1 < w; ++t1) {
+        float pr = 0.0f, pi = 0.0f;
+#pragma unroll
+        for (int t2 = 0; t2 < WMAX; ++t2) {
+            if (t2 < w) {
+                const float *row = base + (size_t)(t1 * sx + t2 * sy) * E;
+                float rr = 0.0f, ri = 0.0f;
+#pragma unroll
+                for (int t3 = 0; t3 < WMAX; ++t3) {
+                    if (t3 < w) {
+                        if (REAL) rr = fmaf(wz[t3], row[t3], rr);
+                        else {
+                            const float2 v = *reinterpret_cast<const float2 *>(row + 2 * t3);
+                            rr = fmaf(wz[t3], v.x, rr);
+                            ri = fmaf(wz[t3], v.y, ri);
+                        }
+                    }
+                }
+                pr = fmaf(wy[t2], rr, pr);
+                if (!REAL) pi = fmaf(wy[t2], ri, pi);
+            }
+        }
+        accr = fmaf(wx[t1], pr, accr);
+        if (!REAL) acci = fmaf(wx[t1], pi, acci);
+    }
+    return make_float2(accr, acci);
+}
+
+template <int OUTK>
+__device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t j, float2 c) {
+    if (OUTK == SPF_OUT_COMPLEX) reinterpret_cast<float2 *>(a.out)[m * a.P + j] = c;
+    else reinterpret_cast<float *>(a.out)[m * a.P + j] = a.scale * c.x;
+}
+
+// W = 0: runtime kernel width (any w <= SPF_MAX_W), else compile-time.
+template <int W, bool REAL, int OUTK, bool STAGED>
+__global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __grid_constant__ SliceArgs a) {
+    constexpr int WMAX = W ? W : SPF_MAX_W;
+    constexpr int E = REAL ? 1 : 2;            // floats per cell
+    constexpr int CELL = 4 * E;                // bytes per cell
+    const int w = W ? W : a.w;
+    const int tid = threadIdx.x;
+    const int64_t m = blockIdx.x / a.n_patches;
+    const int64_t patch = blockIdx.x - m * a.n_patches;
+
+    __shared__ double sR[9];
+    __shared__ int s_lo[3], s_hi[3];
+    __shared__ __align__(8) unsigned long long s_bar;
+    extern __shared__ __align__(128) uint8_t s_tile[];
+
+    if (tid == 0) {
+        quat_to_R(a.quats + 4 * m, sR);
+        s_lo[0] = s_lo[1] = s_lo[2] = INT_MAX;
+        s_hi[0] = s_hi[1] = s_hi[2] = INT_MIN;
+        if (STAGED) { ptx::mbar_init(ptx::smem_u32(&s_bar), 1); ptx::fence_mbar_init(); }
+    }
+    __syncthreads();
+
+    const int64_t j = a.patch[patch * SPF_PATCH + tid];
+    const bool active = (j >= 0);
+    int px = 0, py = 0, pz = 0;
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    if (active) {
+        const double q0 = a.pix_q[3 * j + 0], q1 = a.pix_q[3 * j + 1], q2 = a.pix_q[3 * j + 2];
+        cell_and_fraction(sR[0] * q0 + sR[1] * q1 + sR[2] * q2, a, w, px, fx);
+        cell_and_fraction(sR[3] * q0 + sR[4] * q1 + sR[5] * q2, a, w, py, fy);
+        cell_and_fraction(sR[6] * q0 + sR[7] * q1 + sR[8] * q2, a, w, pz, fz);
+    }
+
+    bool staged = false;
+    int lox = 0, loy = 0, loz = 0, bz = 0, S1 = 0;
+    if (STAGED) {
+        const int lx = __reduce_min_sync(0xffffffffu, active ? px : INT_MAX), hx = __reduce_max_sync(0xffffffffu, active ? px : INT_MIN);
+        const int ly = __reduce_min_sync(0xffffffffu, active ? py : INT_MAX), hy = __reduce_max_sync(0xffffffffu, active ? py : INT_MIN);
+        const int lz = __reduce_min_sync(0xffffffffu, active ? pz : INT_MAX), hz = __reduce_max_sync(0xffffffffu, active ? pz : INT_MIN);
+        if ((tid & 31) == 0) {
+            atomicMin(&s_lo[0], lx); atomicMax(&s_hi[0], hx);
+            atomicMin(&s_lo[1], ly); atomicMax(&s_hi[1], hy);
+            atomicMin(&s_lo[2], lz); atomicMax(&s_hi[2], hz);
+        }
+        __syncthreads();
+        lox = s_lo[0]; loy = s_lo[1]; loz = s_lo[2];
+        const int Lx = s_hi[0] - lox + w, Ly = s_hi[1] - loy + w, Lz = s_hi[2] - loz + w;
+        const int by = max(SPF_BOX_MIN, (Ly + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP);
+        bz = max(SPF_BOX_MIN, (Lz + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP);
+        // x-plane pitch: TMA shared-memory destinations are kept 128-byte aligned
+        S1 = (by * bz + (128 / CELL) - 1) / (128 / CELL) * (128 / CELL);
+        staged = (by <= SPF_BOX_MAX) && (bz <= SPF_BOX_MAX) && ((uint32_t)(Lx * S1 * CELL) <= a.cap_bytes);
+        if (staged && tid < 32) {
+            const uint32_t bar = ptx::smem_u32(&s_bar);
+            if (tid == 0) ptx::mbar_expect_tx(bar, (uint32_t)(Lx * by * bz * CELL));
+            __syncwarp();
+            const CUtensorMap *map = &a.maps.m[((by - SPF_BOX_MIN) / SPF_BOX_STEP) * SPF_BOX_N + (bz - SPF_BOX_MIN) / SPF_BOX_STEP];
+            const uint32_t dst = ptx::smem_u32(s_tile);
+            for (int x = tid; x < Lx; x += 32)
+                ptx::tma_load_3d(dst + (uint32_t)(x * S1 * CELL), map, loz * E, loy, lox + x, bar);
+        }
+    }
+
+    // kernel weights while the tile is in flight
+    float wx[WMAX], wy[WMAX], wz[WMAX];
+    if (STAGED) {
+        weights_poly<WMAX>(fx, w, a, wx); weights_poly<WMAX>(fy, w, a, wy); weights_poly<WMAX>(fz, w, a, wz);
+    } else {
+        weights_direct<WMAX>(fx, w, a.beta, wx); weights_direct<WMAX>(fy, w, a.beta, wy); weights_direct<WMAX>(fz, w, a.beta, wz);
+    }
+
+    float2 c;
+    if (STAGED && staged) {
+        ptx::mbar_wait(ptx::smem_u32(&s_bar), 0);
+        if (!active) return;
+        const float *base = reinterpret_cast<const float *>(s_tile) + (size_t)((px - lox) * S1 + (py - loy) * bz + (pz - loz)) * E;
+        c = gather<WMAX, REAL>(base, S1, bz, w, wx, wy, wz);
+    } else {
+        if (!active) return;
+        const float *base = a.grid + ((size_t)((size_t)px * a.np + py) * a.sz + pz) * E;
+        c = gather<WMAX, REAL>(base, a.np * a.sz, a.sz, w, wx, wy, wz);
+    }
+    store_out<OUTK>(a, m, j, c);
+}
+
+// ------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------
+double es_phi(double z, double beta) { return fabs(z) <= 1.0 ? exp(beta * (sqrt(1.0 - z * z) - 1.0)) : 0.0; }
+
+// per-tap Chebyshev interpolants of phi on the fraction interval, converted to monomials in u
+int fit_kernel_polys(int w, double beta, float coef[SPF_MAX_W][SPF_MAX_DEG + 1]) {
+    for (int deg = 6; deg <= SPF_MAX_DEG; ++deg) {
+        const int n = deg + 1;
+        double worst = 0.0;
+        std::vector<std::vector<double>> mono(w, std::vector<double>(n, 0.0));
+        for (int t = 0; t < w; ++t) {
+            auto g = [&](double u) { return es_phi(((u + 1.0) * 0.5 - 0.5 * w + t) * 2.0 / w, beta); };
+            std::vector<double> cheb(n, 0.0);
+            for (int jn = 0; jn < n; ++jn) {
+                double s = 0.0;
+                for (int k = 0; k < n; ++k) {
+                    const double th = M_PI * (k + 0.5) / n;
+                    s += g(cos(th)) * cos(jn * th);
+                }
+                cheb[jn] = s * (jn == 0 ? 1.0 : 2.0) / n;
+            }
+            // Chebyshev -> monomial: T0 = 1, T1 = u, T_{k+1} = 2 u T_k - T_{k-1}
+            std::vector<double> Tkm1(n, 0.0), Tk(n, 0.0), Tn(n, 0.0);
+            Tkm1[0] = 1.0;
+            for (int i = 0; i < n; ++i) mono[t][i] += cheb[0] * Tkm1[i];
+            if (n > 1) {
+                Tk[1] = 1.0;
+                for (int i = 0; i < n; ++i) mono[t][i] += cheb[1] * Tk[i];
+            }
+            for (int k = 2; k < n; ++k) {
+                for (int i = 0; i < n; ++i) Tn[i] = (i ? 2.0 * Tk[i - 1] : 0.0) - Tkm1[i];
+                for (int i = 0; i < n; ++i) mono[t][i] += cheb[k] * Tn[i];
+                Tkm1 = Tk; Tk = Tn;
+            }
+            for (int s = 0; s < 400; ++s) {
+                const double u = -1.0 + 2.0 * (s + 0.5) / 400.0;
+                double p = mono[t][n - 1];
+                for (int k = n - 2; k >= 0; --k) p = p * u + mono[t][k];
+                worst = fmax(worst, fabs(p - g(u)));
+            }
+        }
+        if (worst < 1e-7 || deg == SPF_MAX_DEG) {
+            for (int t = 0; t < w; ++t)
+                for (int k = 0; k <= SPF_MAX_DEG; ++k) coef[t][k] = k < n ? (float)mono[t][k] : 0.0f;
+            return deg;
+        }
+    }
+    return SPF_MAX_DEG;
+}
+
+// pixel -> patch table: 8 x 16 lattice tiles per panel under a layout promise, else runs of SPF_PATCH pixels
+int build_patches(spf_ctx *ctx, int64_t P) {
+    const bool lattice = ctx->lay_panels > 0 && (int64_t)ctx->lay_panels * ctx->lay_rows * ctx->lay_cols == P;
+    const int key[3] = {lattice ? ctx->lay_panels : 0, lattice ? ctx->lay_rows : 0, lattice ? ctx->lay_cols : 0};
+    if (ctx->d_patch && ctx->patch_P == P && !memcmp(key, ctx->patch_key, sizeof key)) return SPF_OK;
+    std::vector<int32_t> tab;
+    if (lattice) {
+        const int TR = 8, TC = SPF_PATCH / TR;
+        const int R = ctx->lay_rows, C = ctx->lay_cols;
+        for (int p = 0; p < ctx->lay_panels; ++p)
+            for (int r0 = 0; r0 < R; r0 += TR)
+                for (int c0 = 0; c0 < C; c0 += TC)
+                    for (int t = 0; t < SPF_PATCH; ++t) {
+                        const int r = r0 + t / TC, c = c0 + t % TC;
+                        tab.push_back((r < R && c < C) ? (int32_t)(((int64_t)p * R + r) * C + c) : -1);
+                    }
+    } else {
+        const int64_t n = (P + SPF_PATCH - 1) / SPF_PATCH;
+        tab.resize((size_t)n * SPF_PATCH);
+        for (int64_t i = 0; i < n * SPF_PATCH; ++i) tab[(size_t)i] = i < P ? (int32_t)i : -1;
+    }
+    if (ctx->d_patch) { cudaFree(ctx->d_patch); ctx->d_patch = nullptr; }
+    SPF_CUDA(ctx, cudaMalloc(&ctx->d_patch, tab.size() * sizeof(int32_t)));
+    SPF_CUDA(ctx, cudaMemcpy(ctx->d_patch, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    ctx->n_patches = (int64_t)(tab.size() / SPF_PATCH);
+    ctx->patch_P = P;
+    memcpy(ctx->patch_key, key, sizeof key);
+    return SPF_OK;
+}
+
+template <int W, bool REAL, int OUTK, bool STAGED>
+int launch_slice(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, cudaStream_t st) {
+    auto kern = k_slice<W, REAL, OUTK, STAGED>;
+    if (STAGED) SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t blocks = args.n_patches * args.M;
+    if (blocks > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: M * patches exceeds 2^31-1 blocks; split M");
+    kern<<<(unsigned)blocks, SPF_PATCH, STAGED ? smem : 0, st>>>(args);
+    SPF_LAUNCH_CHECK(ctx);
+    return SPF_OK;
+}
+
+template <int W, bool REAL, int OUTK>
+int launch_slice_impl(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, bool staged, cudaStream_t st) {
+    return staged ? launch_slice<W, REAL, OUTK, true>(ctx, args, smem, st) : launch_slice<W, REAL, OUTK, false>(ctx, args, smem, st);
+}
+
+template <bool REAL, int OUTK>
+int launch_slice_w(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, bool staged, cudaStream_t st) {
+    switch (ctx->w) {
+        case 7: return launch_slice_impl<7, REAL, OUTK>(ctx, args, smem, staged, st);
+        case 10: return launch_slice_impl<10, REAL, OUTK>(ctx, args, smem, staged, st);
+        default: return launch_slice<0, REAL, OUTK, false>(ctx, args, smem, st);  // any other width: runtime-w global gather
+    }
+}
+
+}  // namespace
+
+extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const float *pix_q, int64_t P, int32_t out_kind,
+                         float scale, void *out, void *stream_) {
+    if (!ctx) return SPF_EINVAL;
+    if (M < 0 || P < 0) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: negative size");
+    if (out_kind != SPF_OUT_COMPLEX && out_kind != SPF_OUT_INTENSITY) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: bad out_kind %d", out_kind);
+    if (!ctx->prepared) return spf_set_err(ctx, SPF_ESTATE, "spf_slice before spf_prepare_model");
+    if (M == 0 || P == 0) return SPF_OK;
+    if (!quats || !pix_q || !out) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: null pointer");
+    if (P > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: P too large");
+    cudaStream_t st = (cudaStream_t)stream_;
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    int rc = build_patches(ctx, P);
+    if (rc) return rc;
+
+    const bool real = ctx->grid_is_real && !ctx->opt_force_complex;
+    static thread_local SliceArgs args;  // 11 KB: keep it off the stack
+    args.quats = quats; args.pix_q = pix_q; args.patch = ctx->d_patch;
+    args.M = M; args.P = P; args.n_patches = ctx->n_patches;
+    args.out = out; args.scale = scale;
+    args.grid = real ? ctx->d_gridr : reinterpret_cast<const float *>(ctx->d_gridc);
+    args.np = ctx->np; args.sz = ctx->sz; args.off = ctx->nf / 2 + ctx->halo; args.nf = ctx->nf; args.w = ctx->w;
+    args.xi_scale = (double)ctx->nf / (2.0 * M_PI);
+    args.inv_nf = 1.0 / (double)ctx->nf;
+    args.beta = (float)ctx->beta;
+    args.deg = fit_kernel_polys(ctx->w, ctx->beta, args.coef);
+    args.maps = real ? ctx->maps_r : ctx->maps_c;
+    const uint32_t smem = real ? 36u * 1024u : 72u * 1024u;
+    args.cap_bytes = smem;
+    const bool staged = (ctx->opt_slice_impl == 0);
+    if (real) {
+        return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<true, SPF_OUT_COMPLEX>(ctx, args, smem, staged, st)
+                                           : launch_slice_w<true, SPF_OUT_INTENSITY>(ctx, args, smem, staged, st);
+    }
+    return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<false, SPF_OUT_COMPLEX>(ctx, args, smem, staged, st)
+                                       : launch_slice_w<false, SPF_OUT_INTENSITY>(ctx, args, smem, staged, st);
+}
