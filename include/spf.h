@@ -178,6 +178,8 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *   "slice_impl":  [0] shared-memory-staged gather (TMA tile loads); 1 = plain global-memory gather
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
  *   "match_cta_group": [2] CTAs per tcgen05 MMA (2 = cta_group::2 pairs, 1 = single CTA)
+ *   "record_events": [0]; 1 = spf_slice / spf_match record CUDA events on their stream around the
+ *                    dominant kernels, read back with spf_last_kernel_ms
  * Returns SPF_EINVAL for an unknown key or value.
  */
 SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
@@ -187,6 +189,23 @@ SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
  * this library made since the context was created (so the harness can report gpu_launches).
  */
 SPF_API int64_t spf_launch_count(const spf_ctx *ctx);
+
+/*
+ * Device time in milliseconds (CUDA events recorded on the stream the kernel was launched on,
+ * SURVEY.md section 8(d)) of the last call made with option "record_events" = 1:
+ *   which = 0: the interpolation kernel of the last spf_slice   (steps a3-a5, one launch)
+ *   which = 1: the tcgen05 contraction of the last spf_match    (steps a7-a8, both instantiations)
+ *   which = 2: the operand preparation of the last spf_match    (step a6: abs-max, split, norms)
+ * ms [host].  Synchronises on the closing event.  SPF_ESTATE when nothing was recorded.
+ */
+SPF_API int spf_last_kernel_ms(spf_ctx *ctx, int32_t which, float *ms);
+
+/*
+ * Number of fp16 operand products the last spf_match issued per K step: 2 when every image value
+ * was exact in one fp16 term (photon counts), else 3.  products [host].  Synchronises the stream of
+ * that call and reads one word of its workspace, which must still be allocated.
+ */
+SPF_API int spf_last_match_products(spf_ctx *ctx, int32_t *products);
 
 #ifdef __cplusplus
 }

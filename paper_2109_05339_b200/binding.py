@@ -19,7 +19,7 @@ SPF_OUT_INTENSITY = 1
 EXPORTS = ["spf_version", "spf_status_string", "spf_plan_kernel_width", "spf_plan_n_fine", "spf_create", "spf_destroy",
            "spf_get_info", "spf_last_error", "spf_set_detector_layout", "spf_prepare_model", "spf_slice", "spf_match",
            "spf_match_workspace_bytes", "spf_match_reference", "spf_orientation_match_host", "spf_debug_deapodisation",
-           "spf_debug_fine_grid", "spf_set_option", "spf_launch_count"]
+           "spf_debug_fine_grid", "spf_set_option", "spf_launch_count", "spf_last_kernel_ms", "spf_last_match_products"]
 
 
 class SpfParams(C.Structure):
@@ -76,6 +76,8 @@ def load_library():
     lib.spf_set_option.argtypes = [vp, C.c_char_p, i64]
     lib.spf_launch_count.argtypes = [vp]
     lib.spf_launch_count.restype = i64
+    lib.spf_last_kernel_ms.argtypes = [vp, i32, C.POINTER(C.c_float)]
+    lib.spf_last_match_products.argtypes = [vp, C.POINTER(i32)]
     _lib = lib
     return lib
 
@@ -144,6 +146,16 @@ class SpfContext:
 
     def spf_launch_count(self) -> int:
         return int(self._lib.spf_launch_count(self._h))
+
+    def spf_last_kernel_ms(self, which: int) -> float:
+        ms = C.c_float()
+        self._check(self._lib.spf_last_kernel_ms(self._h, which, C.byref(ms)))
+        return float(ms.value)
+
+    def spf_last_match_products(self) -> int:
+        n = C.c_int32()
+        self._check(self._lib.spf_last_match_products(self._h, C.byref(n)))
+        return int(n.value)
 
     def spf_prepare_model(self, model: torch.Tensor):
         n = self.info.n

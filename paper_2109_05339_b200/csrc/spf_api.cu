@@ -93,10 +93,21 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     if (!strcmp(key, "slice_impl") && (value == 0 || value == 1)) { ctx->opt_slice_impl = (int)value; return SPF_OK; }
     if (!strcmp(key, "force_complex_grid") && (value == 0 || value == 1)) { ctx->opt_force_complex = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_cta_group") && (value == 1 || value == 2)) { ctx->opt_match_cta_group = (int)value; return SPF_OK; }
+    if (!strcmp(key, "record_events") && (value == 0 || value == 1)) { ctx->opt_record_events = (int)value; return SPF_OK; }
     return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
 }
 
 int64_t spf_launch_count(const spf_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int spf_last_kernel_ms(spf_ctx *ctx, int32_t which, float *ms) {
+    if (!ctx || !ms) return SPF_EINVAL;
+    if (which < 0 || which > 2) return spf_set_err(ctx, SPF_EINVAL, "spf_last_kernel_ms: which must be 0, 1 or 2");
+    if (!ctx->ev_valid[which]) return spf_set_err(ctx, SPF_ESTATE, "spf_last_kernel_ms: nothing recorded (set option record_events=1 first)");
+    const int a = which == 0 ? 0 : (which == 1 ? 2 : 4), b = which == 0 ? 1 : (which == 1 ? 3 : 2);
+    SPF_CUDA(ctx, cudaEventSynchronize(ctx->ev[b]));
+    SPF_CUDA(ctx, cudaEventElapsedTime(ms, ctx->ev[a], ctx->ev[b]));
+    return SPF_OK;
+}
 
 int spf_orientation_match_host(spf_ctx *ctx, const float *model, const float *quats, int64_t M, const float *pix_q,
                                int64_t P, float scale, const float *images, int64_t n_img, const uint8_t *mask,
@@ -146,6 +157,14 @@ int spf_orientation_match_host(spf_ctx *ctx, const float *model, const float *qu
 }
 
 }  // extern "C"
+
+int spf_record_event(spf_ctx *ctx, int i, cudaStream_t st) {
+    if (!ctx->opt_record_events) return SPF_OK;
+    if (!ctx->ev[0])
+        for (int k = 0; k < 5; ++k) SPF_CUDA(ctx, cudaEventCreate(&ctx->ev[k]));
+    SPF_CUDA(ctx, cudaEventRecord(ctx->ev[i], st));
+    return SPF_OK;
+}
 
 spf_encode_tiled_fn spf_get_encode_tiled() {
     static spf_encode_tiled_fn fn = nullptr;

@@ -36,7 +36,14 @@ struct spf_ctx {
     int opt_slice_impl = 0;
     int opt_force_complex = 0;
     int opt_match_cta_group = 2;
+    int opt_record_events = 0;
     int64_t launches = 0;
+    // CUDA events around the dominant kernels (option "record_events"): [0,1] slice kernel,
+    // [2,3] match GEMM, [4] start of the match operand preparation (which ends at [2])
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid[3] = {false, false, false};
+    const uint32_t *last_scal = nullptr;  // scalars block of the last spf_match's workspace (caller-owned memory)
+    cudaStream_t last_match_stream = nullptr;
 
     std::vector<double> deapod;  // host, n entries
     float *d_deapod = nullptr;   // device fp32 copy (n)
@@ -103,3 +110,5 @@ spf_encode_tiled_fn spf_get_encode_tiled();
 
 // implemented in spf_prepare.cu / spf_slice.cu / spf_match.cu
 int spf_build_slice_maps(spf_ctx *ctx);
+// records ctx->ev[i] on `st` when option "record_events" is on (creates the events on first use)
+int spf_record_event(spf_ctx *ctx, int i, cudaStream_t st);

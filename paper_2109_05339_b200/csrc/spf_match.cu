@@ -420,6 +420,8 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     float *nI = (float *)(ws + L.nI), *nS = (float *)(ws + L.nS);
     __half *plI = (__half *)(ws + L.planesI), *plS = (__half *)(ws + L.planesS);
 
+    int rc;
+    if ((rc = spf_record_event(ctx, 4, st))) return rc;
     SPF_CUDA(ctx, cudaMemsetAsync(scal, 0, 64, st));
     const int rb = ctx->sm_count * 8;
     k_absmax<<<rb, 256, 0, st>>>(images, n_img, P, mask, scal + 0);
@@ -433,7 +435,6 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
 
     const int CG = ctx->opt_match_cta_group;
     CUtensorMap a0, a1, b0, b1;
-    int rc;
     if ((rc = encode_operand_map(ctx, &a0, plI, n_img, L.Ppad, TILE_ROWS))) return rc;
     if ((rc = encode_operand_map(ctx, &a1, plI + (size_t)n_img * L.Ppad, n_img, L.Ppad, TILE_ROWS))) return rc;
     if ((rc = encode_operand_map(ctx, &b0, plS, M, L.Ppad, BN / CG))) return rc;
@@ -444,6 +445,7 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     args.n_mb = (int)((M + BN - 1) / BN);
     args.keys = keys; args.nI = nI; args.nS = nS; args.scal = scal;
     if ((int64_t)args.n_ib * args.n_mb > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: too many tiles");
+    if ((rc = spf_record_event(ctx, 2, st))) return rc;
     if (CG == 2) {
         if ((rc = launch_gemm<2, 1>(ctx, a0, a1, b0, b1, args, st))) return rc;
         if ((rc = launch_gemm<2, 2>(ctx, a0, a1, b0, b1, args, st))) return rc;
@@ -451,8 +453,21 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
         if ((rc = launch_gemm<1, 1>(ctx, a0, a1, b0, b1, args, st))) return rc;
         if ((rc = launch_gemm<1, 2>(ctx, a0, a1, b0, b1, args, st))) return rc;
     }
+    if ((rc = spf_record_event(ctx, 3, st))) return rc;
+    ctx->last_scal = scal; ctx->last_match_stream = st;
+    ctx->ev_valid[1] = ctx->ev_valid[2] = ctx->opt_record_events != 0;
     k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
     SPF_LAUNCH_CHECK(ctx);
+    return SPF_OK;
+}
+
+int spf_last_match_products(spf_ctx *ctx, int32_t *products) {
+    if (!ctx || !products) return SPF_EINVAL;
+    if (!ctx->last_scal) return spf_set_err(ctx, SPF_ESTATE, "spf_last_match_products before spf_match");
+    uint32_t two_planes = 0;
+    SPF_CUDA(ctx, cudaStreamSynchronize(ctx->last_match_stream));
+    SPF_CUDA(ctx, cudaMemcpy(&two_planes, ctx->last_scal + 2, sizeof two_planes, cudaMemcpyDeviceToHost));
+    *products = two_planes ? 3 : 2;
     return SPF_OK;
 }
 

@@ -139,6 +139,8 @@ void spf_destroy(spf_ctx *ctx) {
     if (b.s_main) cudaStreamDestroy(b.s_main);
     if (b.s_copy) cudaStreamDestroy(b.s_copy);
     if (b.ev_img) cudaEventDestroy(b.ev_img);
+    for (int k = 0; k < 5; ++k)
+        if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
     delete ctx;
 }
 

@@ -304,8 +304,12 @@ int launch_slice(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, cudaStream_
     if (STAGED) SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t blocks = args.n_patches * args.M;
     if (blocks > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: M * patches exceeds 2^31-1 blocks; split M");
+    int rc = spf_record_event(ctx, 0, st);
+    if (rc) return rc;
     kern<<<(unsigned)blocks, SPF_PATCH, STAGED ? smem : 0, st>>>(args);
     SPF_LAUNCH_CHECK(ctx);
+    if ((rc = spf_record_event(ctx, 1, st))) return rc;
+    ctx->ev_valid[0] = ctx->opt_record_events != 0;
     return SPF_OK;
 }
 
