@@ -10,37 +10,7 @@
 #include <new>
 
 #include "spf_internal.cuh"
-
-// ------------------------------------------------------------------------------------------
-// host: deapodisation factors in fp64
-// ------------------------------------------------------------------------------------------
-static void gauss_legendre(int n, std::vector<double> &x, std::vector<double> &wgt) {
-    x.resize(n); wgt.resize(n);
-    for (int i = 0; i < (n + 1) / 2; ++i) {
-        double z = cos(M_PI * (i + 0.75) / (n + 0.5)), pp = 0.0;
-        for (int it = 0; it < 100; ++it) {
-            double p1 = 1.0, p2 = 0.0;
-            for (int j = 0; j < n; ++j) { double p3 = p2; p2 = p1; p1 = ((2.0 * j + 1.0) * z * p2 - j * p3) / (j + 1.0); }
-            pp = n * (z * p1 - p2) / (z * z - 1.0);
-            double dz = p1 / pp;
-            z -= dz;
-            if (fabs(dz) < 1e-16) break;
-        }
-        x[i] = -z; x[n - 1 - i] = z;
-        wgt[i] = wgt[n - 1 - i] = 2.0 / ((1.0 - z * z) * pp * pp);
-    }
-}
-
-// phihat(xi) = 2 int_0^1 exp(beta (sqrt(1-z^2) - 1)) cos(xi z) dz; with z = sin(theta) the integrand is analytic:
-//            = 2 int_0^{pi/2} exp(beta (cos(theta) - 1)) cos(xi sin(theta)) cos(theta) dtheta
-static double es_kernel_ft(double xi, double beta, const std::vector<double> &gx, const std::vector<double> &gw) {
-    double s = 0.0;
-    for (size_t k = 0; k < gx.size(); ++k) {
-        double th = 0.25 * M_PI * (gx[k] + 1.0);
-        s += gw[k] * exp(beta * (cos(th) - 1.0)) * cos(xi * sin(th)) * cos(th);
-    }
-    return 2.0 * s * 0.25 * M_PI;
-}
+#include "spf_slice_math.cuh"
 
 // ------------------------------------------------------------------------------------------
 // device kernels
@@ -171,16 +141,9 @@ static int create_impl(spf_ctx *ctx, const spf_params *p) {
     ctx->sm_count = prop.multiProcessorCount;
 
     // deapodisation factors, fp64 on the host
-    std::vector<double> gx, gw;
-    gauss_legendre(96, gx, gw);
-    ctx->deapod.resize(ctx->n);
+    spfm::deapodisation_factors(ctx->n, ctx->nf, ctx->w, ctx->beta, ctx->deapod);
     std::vector<float> p32(ctx->n);
-    const double alpha = M_PI * ctx->w / ctx->nf;
-    for (int i = 0; i < ctx->n; ++i) {
-        double nn = (double)(i - ctx->n / 2);
-        ctx->deapod[i] = 2.0 / (ctx->w * es_kernel_ft(alpha * nn, ctx->beta, gx, gw));
-        p32[i] = (float)ctx->deapod[i];
-    }
+    for (int i = 0; i < ctx->n; ++i) p32[i] = (float)ctx->deapod[i];
     const size_t nf3 = (size_t)ctx->nf * ctx->nf * ctx->nf, ng = (size_t)ctx->np * ctx->np * ctx->sz;
     SPF_CUDA(ctx, cudaMalloc(&ctx->d_deapod, sizeof(float) * ctx->n));
     SPF_CUDA(ctx, cudaMemcpy(ctx->d_deapod, p32.data(), sizeof(float) * ctx->n, cudaMemcpyHostToDevice));

@@ -21,8 +21,7 @@
 
 #include "ptx_sm100.cuh"
 #include "spf_internal.cuh"
-
-#define SPF_MAX_DEG 12
+#include "spf_slice_math.cuh"
 
 namespace {
 
@@ -42,91 +41,9 @@ struct SliceArgs {
     SliceMaps maps;
 };
 
-// rotation matrix of the normalised quaternion, fp64 (reading s2: Hamilton, active)
-__device__ void quat_to_R(const float *q4, double *R) {
-    double w = q4[0], x = q4[1], y = q4[2], z = q4[3];
-    const double inv = 1.0 / sqrt(w * w + x * x + y * y + z * z);
-    w *= inv; x *= inv; y *= inv; z *= inv;
-    R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
-    R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
-    R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
-}
-
-// one axis: rotated coordinate (radians) -> first padded cell index and fraction f = i0 - xi in [-w/2, -w/2 + 1)
-__device__ __forceinline__ void cell_and_fraction(double x, const SliceArgs &a, int w, int &p, float &f) {
-    double xi = x * a.xi_scale;
-    xi -= (double)a.nf * rint(xi * a.inv_nf);  // 2 pi-periodic: fold into [-n_f/2, n_f/2]
-    const double c = ceil(xi - 0.5 * (double)w);
-    p = (int)c + a.off;
-    f = (float)(c - xi);
-}
-
-// weights by the definition (slice_impl = 1): exp(beta (sqrt(1-z^2) - 1)) written as exp(-beta z^2 / (1 + sqrt(1-z^2)))
-template <int WMAX>
-__device__ __forceinline__ void weights_direct(float f, int w, float beta, float (&wt)[WMAX]) {
-    const float s2w = 2.0f / (float)w;
-#pragma unroll
-    for (int t = 0; t < WMAX; ++t) {
-        if (t < w) {
-            const float z = (f + (float)t) * s2w;
-            const float om = fmaxf(fmaf(-z, z, 1.0f), 0.0f);
-            wt[t] = expf(-beta * z * z / (1.0f + sqrtf(om)));
-        }
-    }
-}
-
-// weights by per-tap polynomials in u (Horner, FMA pipe only)
-template <int WMAX>
-__device__ __forceinline__ void weights_poly(float f, int w, const SliceArgs &a, float (&wt)[WMAX]) {
-    const float u = fmaf(2.0f, f, (float)w - 1.0f);  // 2 (f + w/2) - 1
-#pragma unroll
-    for (int t = 0; t < WMAX; ++t) {
-        if (t < w) {
-            float p = a.coef[t][a.deg];
-            for (int k = a.deg - 1; k >= 0; --k) p = fmaf(p, u, a.coef[t][k]);
-            wt[t] = p;
-        }
-    }
-}
-
-// sum over the w^3 neighbours; `base` points at cell (i0x, i0y, i0z), strides in cells
-template <int WMAX, bool REAL>
-__device__ __forceinline__ float2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMAX],
-                                         const float (&wy)[WMAX], const float (&wz)[WMAX]) {
-    float accr = 0.0f, acci = 0.0f;
-    constexpr int E = REAL ? 1 : 2;
-#pragma unroll 1
-    for (int t1 = 0; t1 < w; ++t1) {
-        float pr = 0.0f, pi = 0.0f;
-#pragma unroll
-        for (int t2 = 0; t2 < WMAX; ++t2) {
-            if (t2 < w) {
-                const float *row = base + (size_t)(t1 * sx + t2 * sy) * E;
-                float rr = 0.0f, ri = 0.0f;
-#pragma unroll
-                for (int t3 = 0; t3 < WMAX; ++t3) {
-                    if (t3 < w) {
-                        if (REAL) rr = fmaf(wz[t3], row[t3], rr);
-                        else {
-                            const float2 v = *reinterpret_cast<const float2 *>(row + 2 * t3);
-                            rr = fmaf(wz[t3], v.x, rr);
-                            ri = fmaf(wz[t3], v.y, ri);
-                        }
-                    }
-                }
-                pr = fmaf(wy[t2], rr, pr);
-                if (!REAL) pi = fmaf(wy[t2], ri, pi);
-            }
-        }
-        accr = fmaf(wx[t1], pr, accr);
-        if (!REAL) acci = fmaf(wx[t1], pi, acci);
-    }
-    return make_float2(accr, acci);
-}
-
 template <int OUTK>
-__device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t j, float2 c) {
-    if (OUTK == SPF_OUT_COMPLEX) reinterpret_cast<float2 *>(a.out)[m * a.P + j] = c;
+__device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t j, spfm::c2 c) {
+    if (OUTK == SPF_OUT_COMPLEX) reinterpret_cast<float2 *>(a.out)[m * a.P + j] = make_float2(c.x, c.y);
     else reinterpret_cast<float *>(a.out)[m * a.P + j] = a.scale * c.x;
 }
 
@@ -147,7 +64,7 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
     extern __shared__ __align__(128) uint8_t s_tile[];
 
     if (tid == 0) {
-        quat_to_R(a.quats + 4 * m, sR);
+        spfm::quat_to_R(a.quats + 4 * m, sR);
         s_lo[0] = s_lo[1] = s_lo[2] = INT_MAX;
         s_hi[0] = s_hi[1] = s_hi[2] = INT_MIN;
         if (STAGED) { ptx::mbar_init(ptx::smem_u32(&s_bar), 1); ptx::fence_mbar_init(); }
@@ -160,9 +77,9 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
     float fx = 0.f, fy = 0.f, fz = 0.f;
     if (active) {
         const double q0 = a.pix_q[3 * j + 0], q1 = a.pix_q[3 * j + 1], q2 = a.pix_q[3 * j + 2];
-        cell_and_fraction(sR[0] * q0 + sR[1] * q1 + sR[2] * q2, a, w, px, fx);
-        cell_and_fraction(sR[3] * q0 + sR[4] * q1 + sR[5] * q2, a, w, py, fy);
-        cell_and_fraction(sR[6] * q0 + sR[7] * q1 + sR[8] * q2, a, w, pz, fz);
+        spfm::cell_and_fraction(sR[0] * q0 + sR[1] * q1 + sR[2] * q2, a.xi_scale, a.inv_nf, a.nf, a.off, a.np, w, px, fx);
+        spfm::cell_and_fraction(sR[3] * q0 + sR[4] * q1 + sR[5] * q2, a.xi_scale, a.inv_nf, a.nf, a.off, a.np, w, py, fy);
+        spfm::cell_and_fraction(sR[6] * q0 + sR[7] * q1 + sR[8] * q2, a.xi_scale, a.inv_nf, a.nf, a.off, a.np, w, pz, fz);
     }
 
     bool staged = false;
@@ -198,21 +115,23 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
     // kernel weights while the tile is in flight
     float wx[WMAX], wy[WMAX], wz[WMAX];
     if (STAGED) {
-        weights_poly<WMAX>(fx, w, a, wx); weights_poly<WMAX>(fy, w, a, wy); weights_poly<WMAX>(fz, w, a, wz);
+        spfm::weights_poly<WMAX>(fx, w, a.coef, a.deg, wx); spfm::weights_poly<WMAX>(fy, w, a.coef, a.deg, wy);
+        spfm::weights_poly<WMAX>(fz, w, a.coef, a.deg, wz);
     } else {
-        weights_direct<WMAX>(fx, w, a.beta, wx); weights_direct<WMAX>(fy, w, a.beta, wy); weights_direct<WMAX>(fz, w, a.beta, wz);
+        spfm::weights_direct<WMAX>(fx, w, a.beta, wx); spfm::weights_direct<WMAX>(fy, w, a.beta, wy);
+        spfm::weights_direct<WMAX>(fz, w, a.beta, wz);
     }
 
-    float2 c;
+    spfm::c2 c;
     if (STAGED && staged) {
         ptx::mbar_wait(ptx::smem_u32(&s_bar), 0);
         if (!active) return;
         const float *base = reinterpret_cast<const float *>(s_tile) + (size_t)((px - lox) * S1 + (py - loy) * bz + (pz - loz)) * E;
-        c = gather<WMAX, REAL>(base, S1, bz, w, wx, wy, wz);
+        c = spfm::gather<WMAX, REAL>(base, S1, bz, w, wx, wy, wz);
     } else {
         if (!active) return;
         const float *base = a.grid + ((size_t)((size_t)px * a.np + py) * a.sz + pz) * E;
-        c = gather<WMAX, REAL>(base, a.np * a.sz, a.sz, w, wx, wy, wz);
+        c = spfm::gather<WMAX, REAL>(base, a.np * a.sz, a.sz, w, wx, wy, wz);
     }
     store_out<OUTK>(a, m, j, c);
 }
@@ -220,54 +139,6 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
 // ------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------
-double es_phi(double z, double beta) { return fabs(z) <= 1.0 ? exp(beta * (sqrt(1.0 - z * z) - 1.0)) : 0.0; }
-
-// per-tap Chebyshev interpolants of phi on the fraction interval, converted to monomials in u
-int fit_kernel_polys(int w, double beta, float coef[SPF_MAX_W][SPF_MAX_DEG + 1]) {
-    for (int deg = 6; deg <= SPF_MAX_DEG; ++deg) {
-        const int n = deg + 1;
-        double worst = 0.0;
-        std::vector<std::vector<double>> mono(w, std::vector<double>(n, 0.0));
-        for (int t = 0; t < w; ++t) {
-            auto g = [&](double u) { return es_phi(((u + 1.0) * 0.5 - 0.5 * w + t) * 2.0 / w, beta); };
-            std::vector<double> cheb(n, 0.0);
-            for (int jn = 0; jn < n; ++jn) {
-                double s = 0.0;
-                for (int k = 0; k < n; ++k) {
-                    const double th = M_PI * (k + 0.5) / n;
-                    s += g(cos(th)) * cos(jn * th);
-                }
-                cheb[jn] = s * (jn == 0 ? 1.0 : 2.0) / n;
-            }
-            // Chebyshev -> monomial: T0 = 1, T1 = u, T_{k+1} = 2 u T_k - T_{k-1}
-            std::vector<double> Tkm1(n, 0.0), Tk(n, 0.0), Tn(n, 0.0);
-            Tkm1[0] = 1.0;
-            for (int i = 0; i < n; ++i) mono[t][i] += cheb[0] * Tkm1[i];
-            if (n > 1) {
-                Tk[1] = 1.0;
-                for (int i = 0; i < n; ++i) mono[t][i] += cheb[1] * Tk[i];
-            }
-            for (int k = 2; k < n; ++k) {
-                for (int i = 0; i < n; ++i) Tn[i] = (i ? 2.0 * Tk[i - 1] : 0.0) - Tkm1[i];
-                for (int i = 0; i < n; ++i) mono[t][i] += cheb[k] * Tn[i];
-                Tkm1 = Tk; Tk = Tn;
-            }
-            for (int s = 0; s < 400; ++s) {
-                const double u = -1.0 + 2.0 * (s + 0.5) / 400.0;
-                double p = mono[t][n - 1];
-                for (int k = n - 2; k >= 0; --k) p = p * u + mono[t][k];
-                worst = fmax(worst, fabs(p - g(u)));
-            }
-        }
-        if (worst < 1e-7 || deg == SPF_MAX_DEG) {
-            for (int t = 0; t < w; ++t)
-                for (int k = 0; k <= SPF_MAX_DEG; ++k) coef[t][k] = k < n ? (float)mono[t][k] : 0.0f;
-            return deg;
-        }
-    }
-    return SPF_MAX_DEG;
-}
-
 // pixel -> patch table: 8 x 16 lattice tiles per panel under a layout promise, else runs of SPF_PATCH pixels
 int build_patches(spf_ctx *ctx, int64_t P) {
     const bool lattice = ctx->lay_panels > 0 && (int64_t)ctx->lay_panels * ctx->lay_rows * ctx->lay_cols == P;
@@ -353,7 +224,7 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.xi_scale = (double)ctx->nf / (2.0 * M_PI);
     args.inv_nf = 1.0 / (double)ctx->nf;
     args.beta = (float)ctx->beta;
-    args.deg = fit_kernel_polys(ctx->w, ctx->beta, args.coef);
+    args.deg = spfm::fit_kernel_polys(ctx->w, ctx->beta, args.coef);
     args.maps = real ? ctx->maps_r : ctx->maps_c;
     const uint32_t smem = real ? 36u * 1024u : 72u * 1024u;
     args.cap_bytes = smem;

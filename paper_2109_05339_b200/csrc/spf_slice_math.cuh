@@ -1,0 +1,220 @@
+// Arithmetic of the type-2 NUFFT interpolation (steps a3-a5; PAPER.md:66-68,
+// reading s10), written once for both compilers: nvcc uses these functions inside k_slice and
+// spf_create; tests/hostsim compiles the very same header with g++ so the arithmetic can be checked
+// against the oracle on a box without a GPU.  It is NOT a CPU fallback: nothing in the library's
+// ABI reaches the host versions.
+//
+//   kernel        phi(z) = exp(beta (sqrt(1 - z^2) - 1)) on |z| <= 1,  beta = 2.30 w
+//   point         xi = x n_f / (2 pi) folded into [-n_f/2, n_f/2],  i0 = ceil(xi - w/2),  f = i0 - xi
+//   weights       phi_d[t] = phi(2 (f_d + t) / w),  t = 0..w-1
+//   value         c = sum_{t1,t2,t3} b[i0 + t] phi_1[t1] phi_2[t2] phi_3[t3]
+//   deapodisation p(n) = 2 / (w phihat(pi w n / n_f)),  phihat(xi) = 2 int_0^1 phi(z) cos(xi z) dz
+#pragma once
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include <vector>
+
+#if defined(__CUDACC__)
+#define SPF_HD __host__ __device__ __forceinline__
+#else
+#define SPF_HD inline
+#endif
+
+#ifndef SPF_MAX_W
+#define SPF_MAX_W 16
+#endif
+#define SPF_MAX_DEG 12
+
+namespace spfm {
+
+struct alignas(8) c2 { float x, y; };
+
+// rotation matrix of the normalised quaternion, fp64 (reading s2: (w,x,y,z), Hamilton, active)
+SPF_HD void quat_to_R(const float *q4, double *R) {
+    double w = q4[0], x = q4[1], y = q4[2], z = q4[3];
+    const double inv = 1.0 / sqrt(w * w + x * x + y * y + z * z);
+    w *= inv; x *= inv; y *= inv; z *= inv;
+    R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
+    R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
+    R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
+}
+
+// One axis: rotated coordinate (radians) -> first padded cell index p and fraction f = i0 - xi in
+// [-w/2, -w/2 + 1).  `off` = n_f/2 + halo maps fine cell l to padded index l + off.  The result is
+// clamped to [0, np - w] so that no input (NaN, inf) can index outside the padded grid; for finite
+// input the clamp never acts (lowest index 2, highest n_f + 2).
+SPF_HD void cell_and_fraction(double x, double xi_scale, double inv_nf, int nf, int off, int np, int w, int &p, float &f) {
+    double xi = x * xi_scale;
+    xi -= (double)nf * rint(xi * inv_nf);  // 2 pi-periodic: fold into [-n_f/2, n_f/2]
+    const double c = ceil(xi - 0.5 * (double)w);
+    double fr = c - xi;
+    if (!(fr >= -0.5 * (double)w - 1.0 && fr <= 1.0)) fr = 0.0;   // NaN / inf input
+    double pc = c + (double)off;
+    if (!(pc >= 0.0)) pc = 0.0;
+    if (pc > (double)(np - w)) pc = (double)(np - w);
+    p = (int)pc;
+    f = (float)fr;
+}
+
+// weights by the definition: exp(beta (sqrt(1-z^2) - 1)) written as exp(-beta z^2 / (1 + sqrt(1-z^2)))
+template <int WMAX>
+SPF_HD void weights_direct(float f, int w, float beta, float (&wt)[WMAX]) {
+    const float s2w = 2.0f / (float)w;
+#pragma unroll
+    for (int t = 0; t < WMAX; ++t) {
+        if (t < w) {
+            const float z = (f + (float)t) * s2w;
+            const float om = fmaxf(fmaf(-z, z, 1.0f), 0.0f);
+            wt[t] = expf(-beta * z * z / (1.0f + sqrtf(om)));
+        }
+    }
+}
+
+// weights by per-tap polynomials in u = 2 (f + w/2) - 1 in [-1, 1) (Horner, FMA pipe only);
+// coef[t][k] from fit_kernel_polys
+template <int WMAX>
+SPF_HD void weights_poly(float f, int w, const float (*coef)[SPF_MAX_DEG + 1], int deg, float (&wt)[WMAX]) {
+    const float u = fmaf(2.0f, f, (float)w - 1.0f);
+#pragma unroll
+    for (int t = 0; t < WMAX; ++t) {
+        if (t < w) {
+            float p = coef[t][deg];
+            for (int k = deg - 1; k >= 0; --k) p = fmaf(p, u, coef[t][k]);
+            wt[t] = p;
+        }
+    }
+}
+
+// sum over the w^3 neighbours; `base` points at cell (i0x, i0y, i0z); sx, sy strides in cells
+template <int WMAX, bool REAL>
+SPF_HD c2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMAX], const float (&wy)[WMAX],
+                 const float (&wz)[WMAX]) {
+    float accr = 0.0f, acci = 0.0f;
+    constexpr int E = REAL ? 1 : 2;
+#pragma unroll 1
+    for (int t1 = 0; t1 < w; ++t1) {
+        float pr = 0.0f, pi = 0.0f;
+#pragma unroll
+        for (int t2 = 0; t2 < WMAX; ++t2) {
+            if (t2 < w) {
+                const float *row = base + (size_t)(t1 * sx + t2 * sy) * E;
+                float rr = 0.0f, ri = 0.0f;
+#pragma unroll
+                for (int t3 = 0; t3 < WMAX; ++t3) {
+                    if (t3 < w) {
+                        if (REAL) rr = fmaf(wz[t3], row[t3], rr);
+                        else {
+                            const c2 v = *reinterpret_cast<const c2 *>(row + 2 * t3);  // one 64-bit load
+                            rr = fmaf(wz[t3], v.x, rr);
+                            ri = fmaf(wz[t3], v.y, ri);
+                        }
+                    }
+                }
+                pr = fmaf(wy[t2], rr, pr);
+                if (!REAL) pi = fmaf(wy[t2], ri, pi);
+            }
+        }
+        accr = fmaf(wx[t1], pr, accr);
+        if (!REAL) acci = fmaf(wx[t1], pi, acci);
+    }
+    c2 r; r.x = accr; r.y = acci;
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------
+// host side (fp64): kernel, polynomial fit of the weights, deapodisation factors
+// ------------------------------------------------------------------------------------------
+inline double es_phi(double z, double beta) { return fabs(z) <= 1.0 ? exp(beta * (sqrt(1.0 - z * z) - 1.0)) : 0.0; }
+
+// Per-tap Chebyshev interpolants of phi on the fraction interval, converted to monomials in u.
+// Returns the degree used: the lowest in [6, SPF_MAX_DEG] whose worst error over all taps is < 1e-7.
+inline int fit_kernel_polys(int w, double beta, float coef[SPF_MAX_W][SPF_MAX_DEG + 1], double *worst_out = nullptr) {
+    const double kPi = 3.14159265358979323846;
+    for (int deg = 6; deg <= SPF_MAX_DEG; ++deg) {
+        const int n = deg + 1;
+        double worst = 0.0;
+        std::vector<std::vector<double>> mono(w, std::vector<double>(n, 0.0));
+        for (int t = 0; t < w; ++t) {
+            auto g = [&](double u) { return es_phi(((u + 1.0) * 0.5 - 0.5 * w + t) * 2.0 / w, beta); };
+            std::vector<double> cheb(n, 0.0);
+            for (int jn = 0; jn < n; ++jn) {
+                double s = 0.0;
+                for (int k = 0; k < n; ++k) {
+                    const double th = kPi * (k + 0.5) / n;
+                    s += g(cos(th)) * cos(jn * th);
+                }
+                cheb[jn] = s * (jn == 0 ? 1.0 : 2.0) / n;
+            }
+            // Chebyshev -> monomial: T0 = 1, T1 = u, T_{k+1} = 2 u T_k - T_{k-1}
+            std::vector<double> Tkm1(n, 0.0), Tk(n, 0.0), Tn(n, 0.0);
+            Tkm1[0] = 1.0;
+            for (int i = 0; i < n; ++i) mono[t][i] += cheb[0] * Tkm1[i];
+            if (n > 1) {
+                Tk[1] = 1.0;
+                for (int i = 0; i < n; ++i) mono[t][i] += cheb[1] * Tk[i];
+            }
+            for (int k = 2; k < n; ++k) {
+                for (int i = 0; i < n; ++i) Tn[i] = (i ? 2.0 * Tk[i - 1] : 0.0) - Tkm1[i];
+                for (int i = 0; i < n; ++i) mono[t][i] += cheb[k] * Tn[i];
+                Tkm1 = Tk; Tk = Tn;
+            }
+            for (int s = 0; s < 400; ++s) {
+                const double u = -1.0 + 2.0 * (s + 0.5) / 400.0;
+                double p = mono[t][n - 1];
+                for (int k = n - 2; k >= 0; --k) p = p * u + mono[t][k];
+                worst = fmax(worst, fabs(p - g(u)));
+            }
+        }
+        if (worst < 1e-7 || deg == SPF_MAX_DEG) {
+            for (int t = 0; t < w; ++t)
+                for (int k = 0; k <= SPF_MAX_DEG; ++k) coef[t][k] = k < n ? (float)mono[t][k] : 0.0f;
+            if (worst_out) *worst_out = worst;
+            return deg;
+        }
+    }
+    return SPF_MAX_DEG;
+}
+
+inline void gauss_legendre(int n, std::vector<double> &x, std::vector<double> &wgt) {
+    const double kPi = 3.14159265358979323846;
+    x.resize(n); wgt.resize(n);
+    for (int i = 0; i < (n + 1) / 2; ++i) {
+        double z = cos(kPi * (i + 0.75) / (n + 0.5)), pp = 0.0;
+        for (int it = 0; it < 100; ++it) {
+            double p1 = 1.0, p2 = 0.0;
+            for (int j = 0; j < n; ++j) { double p3 = p2; p2 = p1; p1 = ((2.0 * j + 1.0) * z * p2 - j * p3) / (j + 1.0); }
+            pp = n * (z * p1 - p2) / (z * z - 1.0);
+            double dz = p1 / pp;
+            z -= dz;
+            if (fabs(dz) < 1e-16) break;
+        }
+        x[i] = -z; x[n - 1 - i] = z;
+        wgt[i] = wgt[n - 1 - i] = 2.0 / ((1.0 - z * z) * pp * pp);
+    }
+}
+
+// phihat(xi) = 2 int_0^1 exp(beta (sqrt(1-z^2) - 1)) cos(xi z) dz; with z = sin(theta) the integrand is analytic:
+//            = 2 int_0^{pi/2} exp(beta (cos(theta) - 1)) cos(xi sin(theta)) cos(theta) dtheta
+inline double es_kernel_ft(double xi, double beta, const std::vector<double> &gx, const std::vector<double> &gw) {
+    const double kPi = 3.14159265358979323846;
+    double s = 0.0;
+    for (size_t k = 0; k < gx.size(); ++k) {
+        double th = 0.25 * kPi * (gx[k] + 1.0);
+        s += gw[k] * exp(beta * (cos(th) - 1.0)) * cos(xi * sin(th)) * cos(th);
+    }
+    return 2.0 * s * 0.25 * kPi;
+}
+
+// p(n) for n = i - floor(N/2), i = 0..N-1
+inline void deapodisation_factors(int N, int nf, int w, double beta, std::vector<double> &out) {
+    const double kPi = 3.14159265358979323846;
+    std::vector<double> gx, gw;
+    gauss_legendre(96, gx, gw);
+    out.resize(N);
+    const double alpha = kPi * w / nf;
+    for (int i = 0; i < N; ++i) out[i] = 2.0 / (w * es_kernel_ft(alpha * (double)(i - N / 2), beta, gx, gw));
+}
+
+}  // namespace spfm
