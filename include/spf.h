@@ -55,7 +55,8 @@ typedef enum {
     SPF_EINVAL = -1, /* bad size, null pointer, unsupported parameter (checked on host-side arguments only) */
     SPF_ENOMEM = -2, /* host or device allocation failed */
     SPF_ECUDA = -3,  /* a CUDA / cuFFT / driver call failed; text in spf_last_error */
-    SPF_ESTATE = -4  /* call order: spf_slice before spf_prepare_model */
+    SPF_ESTATE = -4, /* call order: spf_slice before spf_prepare_model */
+    SPF_EFAULT = -5  /* a kernel's pipeline watchdog gave up (see spf_check_fault); results of that call are invalid */
 } spf_status;
 
 typedef struct spf_ctx spf_ctx; /* opaque */
@@ -174,15 +175,28 @@ SPF_API int spf_debug_deapodisation(const spf_ctx *ctx, double *out_host);
 SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stream);
 
 /*
- * Test/benchmark knobs (defaults in brackets):
- *   "slice_impl":  [0] shared-memory-staged gather (TMA tile loads); 1 = plain global-memory gather
+ * Kernel variants and test/benchmark knobs (defaults in brackets):
+ *   "slice_impl":  0 = shared-memory-staged gather (TMA tile loads); [1] = plain global-memory gather
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
- *   "match_cta_group": [2] CTAs per tcgen05 MMA (2 = cta_group::2 pairs, 1 = single CTA)
+ *   "match_cta_group": CTAs per tcgen05 MMA: 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
+ * The defaults are the variants with the least machinery; the faster ones (0 and 2) are switched
+ * on by the caller once they have been checked on the device at hand (the Python binding's
+ * SpfContext.spf_autotune does that in a child process).
  *   "record_events": [0]; 1 = spf_slice / spf_match record CUDA events on their stream around the
  *                    dominant kernels, read back with spf_last_kernel_ms
  * Returns SPF_EINVAL for an unknown key or value.
  */
 SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
+
+/*
+ * Watchdog.  Every wait on a hardware barrier inside the slicing and matching kernels is bounded
+ * (about two seconds of SM clocks): a pipeline that stalls makes its block record a fault and
+ * leave through the normal teardown instead of spinning for ever.  spf_check_fault synchronises
+ * `stream`, and returns SPF_EFAULT (text: which kernel, role, block and tile) if any kernel
+ * launched through this context since the last check recorded one, else SPF_OK.  The fault is
+ * cleared by the call.  spf_orientation_match_host checks it itself before returning.
+ */
+SPF_API int spf_check_fault(spf_ctx *ctx, void *stream);
 
 /*
  * Device-time statistics of the last spf_slice / spf_match, for bench.py: counts of launches

@@ -19,7 +19,8 @@ SPF_OUT_INTENSITY = 1
 EXPORTS = ["spf_version", "spf_status_string", "spf_plan_kernel_width", "spf_plan_n_fine", "spf_create", "spf_destroy",
            "spf_get_info", "spf_last_error", "spf_set_detector_layout", "spf_prepare_model", "spf_slice", "spf_match",
            "spf_match_workspace_bytes", "spf_match_reference", "spf_orientation_match_host", "spf_debug_deapodisation",
-           "spf_debug_fine_grid", "spf_set_option", "spf_launch_count", "spf_last_kernel_ms", "spf_last_match_products"]
+           "spf_debug_fine_grid", "spf_set_option", "spf_launch_count", "spf_last_kernel_ms", "spf_last_match_products",
+           "spf_check_fault"]
 
 
 class SpfParams(C.Structure):
@@ -78,6 +79,7 @@ def load_library():
     lib.spf_launch_count.restype = i64
     lib.spf_last_kernel_ms.argtypes = [vp, i32, C.POINTER(C.c_float)]
     lib.spf_last_match_products.argtypes = [vp, C.POINTER(i32)]
+    lib.spf_check_fault.argtypes = [vp, vp]
     _lib = lib
     return lib
 
@@ -143,6 +145,20 @@ class SpfContext:
 
     def spf_set_option(self, key: str, value: int):
         self._check(self._lib.spf_set_option(self._h, key.encode(), int(value)))
+
+    def spf_check_fault(self):
+        """Synchronise the current stream; raise SpfError(SPF_EFAULT) if a kernel's watchdog gave up."""
+        self._check(self._lib.spf_check_fault(self._h, _stream(self.device)))
+
+    def spf_autotune(self, timeout_s: float = 240.0) -> dict:
+        """Switch on the faster kernel variants (TMA-staged slicing, cta_group::2 matching) that pass the
+        device self-check (selfcheck.py, run once per process in a child process so that a faulting
+        variant cannot take this process's CUDA context with it).  Returns {variant: bool}."""
+        from .selfcheck import verified_variants
+        ok = verified_variants(self.device.index or 0, timeout_s)
+        self.spf_set_option("slice_impl", 0 if ok.get("slice_staged") else 1)
+        self.spf_set_option("match_cta_group", 2 if ok.get("match_cg2") else 1)
+        return ok
 
     def spf_launch_count(self) -> int:
         return int(self._lib.spf_launch_count(self._h))

@@ -47,9 +47,29 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    while (!mbar_try_wait(bar, parity)) {
+// Bounded wait, executed by a whole (converged) warp.  Every wait in libspf is satisfied within
+// microseconds when the pipeline is correct; a wait that lasts SPF_WAIT_CYCLES (about 2 s) means the
+// pipeline is broken, and spinning for ever would take the GPU down with it.  So the wait gives up:
+// it raises the block's abort word in shared memory (every other wait of the block then gives up at
+// its next poll) and returns false.  The caller records the fault in the context's fault word and
+// leaves through the kernel's normal teardown; the host reports SPF_ECUDA at its next check.
+#ifndef SPF_WAIT_CYCLES
+#define SPF_WAIT_CYCLES (1ll << 32)
+#endif
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t *abort_word) {
+    bool ok = mbar_try_wait(bar, parity);
+    if (!ok) {
+        const long long t0 = clock64();
+        uint32_t polls = 0;
+        for (;;) {
+            if (mbar_try_wait(bar, parity)) { ok = true; break; }
+            if ((++polls & 63u) == 0) {
+                if (*abort_word) break;
+                if (clock64() - t0 > SPF_WAIT_CYCLES) { *abort_word = 1u; break; }
+            }
+        }
     }
+    return __all_sync(0xffffffffu, ok);
 }
 
 // ---------------------------------------------------------------- TMA

@@ -41,6 +41,7 @@ const char *spf_status_string(int s) {
         case SPF_ENOMEM: return "SPF_ENOMEM";
         case SPF_ECUDA: return "SPF_ECUDA";
         case SPF_ESTATE: return "SPF_ESTATE";
+        case SPF_EFAULT: return "SPF_EFAULT";
         default: return "SPF_UNKNOWN";
     }
 }
@@ -95,6 +96,22 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     if (!strcmp(key, "match_cta_group") && (value == 1 || value == 2)) { ctx->opt_match_cta_group = (int)value; return SPF_OK; }
     if (!strcmp(key, "record_events") && (value == 0 || value == 1)) { ctx->opt_record_events = (int)value; return SPF_OK; }
     return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
+}
+
+int spf_check_fault(spf_ctx *ctx, void *stream_) {
+    if (!ctx) return SPF_EINVAL;
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    SPF_CUDA(ctx, cudaStreamSynchronize((cudaStream_t)stream_));
+    if (!ctx->h_fault || ctx->h_fault[0] == 0u) return SPF_OK;
+    const uint32_t code = ctx->h_fault[0], block = ctx->h_fault[1], unit = ctx->h_fault[2], variant = ctx->h_fault[3];
+    ctx->h_fault[0] = ctx->h_fault[1] = ctx->h_fault[2] = ctx->h_fault[3] = 0u;
+    if (code >= SPF_FAULT_MATCH) {
+        static const char *role[4] = {"TMA producer (slot never freed)", "MMA issuer (accumulator never drained)",
+                                      "MMA issuer (operands never arrived)", "epilogue (accumulator never completed)"};
+        return spf_set_err(ctx, SPF_EFAULT, "watchdog: k_match_gemm<CG=%u,NI=%u> %s, block %u, tile %u", variant / 10, variant % 10,
+                           role[(code - SPF_FAULT_MATCH) & 3u], block, unit);
+    }
+    return spf_set_err(ctx, SPF_EFAULT, "watchdog: k_slice (variant %u) tile never arrived, block %u", variant, block);
 }
 
 int64_t spf_launch_count(const spf_ctx *ctx) { return ctx ? ctx->launches : 0; }
@@ -152,8 +169,7 @@ int spf_orientation_match_host(spf_ctx *ctx, const float *model, const float *qu
     SPF_CUDA(ctx, cudaMemcpyAsync(best_dist, b.bdist, (size_t)n_img * 4, cudaMemcpyDeviceToHost, b.s_main));
     if (slices_out)
         SPF_CUDA(ctx, cudaMemcpyAsync(slices_out, b.slices, (size_t)M * P * 4, cudaMemcpyDeviceToHost, b.s_main));
-    SPF_CUDA(ctx, cudaStreamSynchronize(b.s_main));
-    return SPF_OK;
+    return spf_check_fault(ctx, b.s_main);
 }
 
 }  // extern "C"

@@ -33,9 +33,9 @@ struct spf_ctx {
     int sm_count = 0;
     bool prepared = false;
     bool grid_is_real = false;
-    int opt_slice_impl = 0;
+    int opt_slice_impl = 1;       // conservative defaults until a variant has been checked on the device (spf.h)
     int opt_force_complex = 0;
-    int opt_match_cta_group = 2;
+    int opt_match_cta_group = 1;
     int opt_record_events = 0;
     int64_t launches = 0;
     // CUDA events around the dominant kernels (option "record_events"): [0,1] slice kernel,
@@ -77,8 +77,16 @@ struct spf_ctx {
         cudaEvent_t ev_img = nullptr;
     } hb;
 
+    // watchdog fault record: 4 words of pinned, device-mapped host memory
+    // [0] code (0 = none), [1] block, [2] tile / patch, [3] kernel variant
+    volatile uint32_t *h_fault = nullptr;
+    uint32_t *d_fault = nullptr;
+
     std::string err;
 };
+
+#define SPF_FAULT_SLICE 16u  // k_slice: tile wait gave up
+#define SPF_FAULT_MATCH 32u  // k_match_gemm: + 0 producer, 1 MMA (accumulator), 2 MMA (operands), 3 epilogue
 
 #define SPF_PATCH 128  // threads per slicing block = pixels per patch
 

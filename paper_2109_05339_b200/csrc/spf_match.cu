@@ -28,7 +28,7 @@ constexpr int A_TILE_BYTES = TILE_ROWS * BK * 2;  // 16 KB
 constexpr int GEMM_THREADS = 192;                 // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
 constexpr int ACC_STAGES = 2;
 constexpr int TMEM_COLS = ACC_STAGES * BN;        // 512: all of TMEM, one CTA per SM
-constexpr size_t SMEM_AUX = 4096;                 // barriers, tmem pointer, ||S||^2 tile buffers
+constexpr size_t SMEM_AUX = 6144;                 // 1 KB barriers, tmem pointer, abort word; 4 KB per-warp ||S||^2 tiles
 constexpr size_t SMEM_BUDGET = 227 * 1024;
 
 template <int CG, int NI>
@@ -49,6 +49,7 @@ struct MatchArgs {
     unsigned long long *keys;
     const float *nI, *nS;
     const uint32_t *scal;   // [2] = image plane 2 needed, [4] = eI, [5] = eS
+    uint32_t *fault;        // context fault word (host-mapped): written when a pipeline wait gives up
 };
 
 struct WsLayout {
@@ -177,7 +178,8 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     uint8_t *aux_p = smem_al + (size_t)ST * Cfg::STAGE_BYTES;
     const uint32_t bar_full = aux, bar_empty = aux + 8 * ST, bar_tfull = aux + 16 * ST, bar_tempty = bar_tfull + 8 * ACC_STAGES;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(aux_p + 16 * ST + 16 * ACC_STAGES);
-    float *nsbuf = reinterpret_cast<float *>(aux_p + 1024);  // [ACC_STAGES][BN]
+    volatile uint32_t *abort_w = tmem_slot + 1;              // raised by the first wait that gives up
+    float *nsbuf = reinterpret_cast<float *>(aux_p + 1024);  // [4 epilogue warps][BN]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
@@ -186,6 +188,7 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     const int n_tiles = a.n_ib * a.n_mb;
 
     if (warp == 0 && lane == 0) {
+        *abort_w = 0u;
         ptx::prefetch_tensormap(&mapA0); ptx::prefetch_tensormap(&mapB0); ptx::prefetch_tensormap(&mapB1);
         if (NI == 2) ptx::prefetch_tensormap(&mapA1);
         for (int s = 0; s < ST; ++s) { ptx::mbar_init(bar_full + 8 * s, 1); ptx::mbar_init(bar_empty + 8 * s, 1); }
@@ -209,15 +212,25 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
         mb = r / gsz;
     };
 
+    // a wait that gave up: note where (first writer wins is not needed -- any one record will do)
+    auto give_up = [&](uint32_t role, int t) {
+        if (lane == 0) {
+            a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)t; a.fault[3] = (uint32_t)(CG * 10 + NI);
+            a.fault[0] = SPF_FAULT_MATCH + role;
+            __threadfence_system();
+        }
+    };
+
     if (warp == 0) {
         // ===================== TMA producer =====================
         int s = 0; uint32_t ph = 0;
-        for (int t = cluster_id; t < n_tiles; t += n_clusters) {
+        bool alive = true;
+        for (int t = cluster_id; alive && t < n_tiles; t += n_clusters) {
             int ib, mb; tile_coords(t, ib, mb);
             const int rowA = ib * (TILE_ROWS * CG) + (int)rank * TILE_ROWS;
             const int rowB = mb * BN + (int)rank * Cfg::B_ROWS;
             for (int kb = 0; kb < a.kblocks; ++kb) {
-                ptx::mbar_wait(bar_empty + 8 * s, ph ^ 1u);
+                if (!ptx::mbar_wait(bar_empty + 8 * s, ph ^ 1u, abort_w)) { give_up(0, t); alive = false; break; }
                 if (lane == 0) {
                     const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
                     const uint32_t fb = bar_full + 8 * s;
@@ -245,12 +258,14 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
         if (leader) {
             constexpr uint32_t idesc = ptx::umma_idesc_f16(TILE_ROWS * CG, BN);
             int s = 0; uint32_t ph = 0; int as = 0; uint32_t aph = 0;
-            for (int t = cluster_id; t < n_tiles; t += n_clusters) {
-                ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u);  // epilogue has drained this accumulator stage
+            bool alive = true;
+            for (int t = cluster_id; alive && t < n_tiles; t += n_clusters) {
+                // epilogue has drained this accumulator stage
+                if (!ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u, abort_w)) { give_up(1, t); break; }
                 ptx::tc_fence_after();
                 const uint32_t tacc = tmem_base + (uint32_t)(as * BN);
                 for (int kb = 0; kb < a.kblocks; ++kb) {
-                    ptx::mbar_wait(bar_full + 8 * s, ph);
+                    if (!ptx::mbar_wait(bar_full + 8 * s, ph, abort_w)) { give_up(2, t); alive = false; break; }
                     ptx::tc_fence_after();
                     if (lane == 0) {
                         const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
@@ -276,19 +291,21 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
         }
     } else {
         // ===================== epilogue: TMEM -> registers -> norm add + running argmin =====================
+        // Each warp works alone (its own TMEM lane quadrant, its own copy of the tile's ||S||^2), so
+        // the four warps never wait for one another.
         const int q = warp & 3;                 // TMEM lane quadrant this warp may read
-        const int e = (warp - 2) * 32 + lane;   // 0..127 among the epilogue threads
+        float *nsb = nsbuf + (warp - 2) * BN;
         const float neg2sc = ldexpf(-2.0f, -((int)a.scal[4] + (int)a.scal[5]));
         int as = 0; uint32_t aph = 0;
         for (int t = cluster_id; t < n_tiles; t += n_clusters) {
             int ib, mb; tile_coords(t, ib, mb);
             const int64_t m0 = (int64_t)mb * BN;
-            float *nsb = nsbuf + as * BN;
-            for (int k = e; k < BN; k += 128) nsb[k] = (m0 + k < a.M) ? a.nS[m0 + k] : INFINITY;
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            __syncwarp();
+            for (int k = lane; k < BN; k += 32) nsb[k] = (m0 + k < a.M) ? a.nS[m0 + k] : INFINITY;
+            __syncwarp();
             const int64_t i = (int64_t)ib * (TILE_ROWS * CG) + (int64_t)rank * TILE_ROWS + q * 32 + lane;
             const float nIv = (i < a.n_img) ? a.nI[i] : 0.0f;
-            ptx::mbar_wait(bar_tfull + 8 * as, aph);
+            if (!ptx::mbar_wait(bar_tfull + 8 * as, aph, abort_w)) { give_up(3, t); break; }
             ptx::tc_fence_after();
             float best = INFINITY; uint32_t bm = 0xffffffffu;
             const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * BN);
@@ -443,7 +460,7 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     args.n_img = n_img; args.M = M; args.kblocks = (int)(L.Ppad / BK);
     args.n_ib = (int)((n_img + TILE_ROWS * CG - 1) / (TILE_ROWS * CG));
     args.n_mb = (int)((M + BN - 1) / BN);
-    args.keys = keys; args.nI = nI; args.nS = nS; args.scal = scal;
+    args.keys = keys; args.nI = nI; args.nS = nS; args.scal = scal; args.fault = ctx->d_fault;
     if ((int64_t)args.n_ib * args.n_mb > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: too many tiles");
     if ((rc = spf_record_event(ctx, 2, st))) return rc;
     if (CG == 2) {

@@ -103,6 +103,7 @@ void spf_destroy(spf_ctx *ctx) {
     if (ctx->plan_ok) cufftDestroy(ctx->plan);
     cudaFree(ctx->d_deapod); cudaFree(ctx->d_fft); cudaFree(ctx->d_gridc); cudaFree(ctx->d_gridr);
     cudaFree(ctx->d_flag); cudaFree(ctx->d_patch);
+    if (ctx->h_fault) cudaFreeHost((void *)ctx->h_fault);
     auto &b = ctx->hb;
     cudaFree(b.model); cudaFree(b.quats); cudaFree(b.pix); cudaFree(b.images); cudaFree(b.slices);
     cudaFree(b.mask); cudaFree(b.bidx); cudaFree(b.bdist); cudaFree(b.ws);
@@ -151,6 +152,11 @@ static int create_impl(spf_ctx *ctx, const spf_params *p) {
     SPF_CUDA(ctx, cudaMalloc(&ctx->d_gridc, sizeof(float2) * ng));
     SPF_CUDA(ctx, cudaMalloc(&ctx->d_gridr, sizeof(float) * ng));
     SPF_CUDA(ctx, cudaMalloc(&ctx->d_flag, sizeof(int)));
+    void *hf = nullptr;
+    SPF_CUDA(ctx, cudaHostAlloc(&hf, 4 * sizeof(uint32_t), cudaHostAllocMapped));
+    memset(hf, 0, 4 * sizeof(uint32_t));
+    ctx->h_fault = (volatile uint32_t *)hf;
+    SPF_CUDA(ctx, cudaHostGetDevicePointer((void **)&ctx->d_fault, hf, 0));
     cufftResult fr = cufftPlan3d(&ctx->plan, ctx->nf, ctx->nf, ctx->nf, CUFFT_C2C);
     if (fr != CUFFT_SUCCESS) return spf_set_err(ctx, fr == CUFFT_ALLOC_FAILED ? SPF_ENOMEM : SPF_ECUDA, "cufftPlan3d(%d^3) failed: %d", ctx->nf, (int)fr);
     ctx->plan_ok = true;

@@ -37,6 +37,7 @@ struct SliceArgs {
     double inv_nf;
     float beta;
     uint32_t cap_bytes;     // dynamic shared memory available for the tile
+    uint32_t *fault;        // context fault word (host-mapped): written when the tile wait gives up
     float coef[SPF_MAX_W][SPF_MAX_DEG + 1];  // phi at tap t as a polynomial in u = 2 (f + w/2) - 1
     SliceMaps maps;
 };
@@ -61,13 +62,14 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
     __shared__ double sR[9];
     __shared__ int s_lo[3], s_hi[3];
     __shared__ __align__(8) unsigned long long s_bar;
+    __shared__ uint32_t s_abort;
     extern __shared__ __align__(128) uint8_t s_tile[];
 
     if (tid == 0) {
         spfm::quat_to_R(a.quats + 4 * m, sR);
         s_lo[0] = s_lo[1] = s_lo[2] = INT_MAX;
         s_hi[0] = s_hi[1] = s_hi[2] = INT_MIN;
-        if (STAGED) { ptx::mbar_init(ptx::smem_u32(&s_bar), 1); ptx::fence_mbar_init(); }
+        if (STAGED) { s_abort = 0u; ptx::mbar_init(ptx::smem_u32(&s_bar), 1); ptx::fence_mbar_init(); }
     }
     __syncthreads();
 
@@ -124,7 +126,14 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
 
     spfm::c2 c;
     if (STAGED && staged) {
-        ptx::mbar_wait(ptx::smem_u32(&s_bar), 0);
+        if (!ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort)) {
+            if (tid == 0) {
+                a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)patch; a.fault[3] = (uint32_t)(W * 10 + (REAL ? 1 : 0));
+                a.fault[0] = SPF_FAULT_SLICE;
+                __threadfence_system();
+            }
+            return;
+        }
         if (!active) return;
         const float *base = reinterpret_cast<const float *>(s_tile) + (size_t)((px - lox) * S1 + (py - loy) * bz + (pz - loz)) * E;
         c = spfm::gather<WMAX, REAL>(base, S1, bz, w, wx, wy, wz);
@@ -228,6 +237,7 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.maps = real ? ctx->maps_r : ctx->maps_c;
     const uint32_t smem = real ? 36u * 1024u : 72u * 1024u;
     args.cap_bytes = smem;
+    args.fault = ctx->d_fault;
     const bool staged = (ctx->opt_slice_impl == 0);
     if (real) {
         return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<true, SPF_OUT_COMPLEX>(ctx, args, smem, staged, st)

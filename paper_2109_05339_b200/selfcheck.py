@@ -1,0 +1,159 @@
+"""Device self-check of libspf's kernel variants.
+
+libspf has two implementations of each hot kernel: one with the least machinery (plain global
+gather; single-CTA tcgen05 GEMM) and a faster one (TMA-staged shared-memory gather; cta_group::2
+GEMM on CTA pairs).  The library starts on the first; `SpfContext.spf_autotune()` switches on the
+second where this self-check passes on the device at hand.
+
+A check runs in a CHILD process (`python -m paper_2109_05339_b200.selfcheck <variant>`): a kernel
+that faults poisons its CUDA context, and the caller's must survive that.  The child compares the
+variant with another computation made by the library's own kernels on the same device -- the
+staged gather with the global gather, the tensor-core matcher with the CUDA-core difference-form
+matcher (`spf_match_reference`) -- on seeded random inputs that span several tiles and a ragged
+tail.  This is a consistency check between two CUDA paths, not parity: parity against the oracle
+is what tests/ does.  Nothing here touches `oracle/`.
+
+Exit status of the child: 0 = variant agrees, 1 = disagrees or raised, anything else (signal,
+time-out) = faulted.
+"""
+import json
+import os
+import subprocess
+import sys
+import time
+
+VARIANTS = ("match_cg1", "slice_staged", "match_cg2")
+_ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+_cache = {}
+
+
+def _check_slice_staged(device: int) -> str:
+    import torch
+    from .binding import SpfContext, SPF_OUT_COMPLEX
+    dev = torch.device("cuda", device)
+    g = torch.Generator(device="cpu"); g.manual_seed(11)
+    worst = 0.0
+    for n, eps, even in ((24, 1e-6, True), (21, 1e-6, False), (20, 1e-9, True)):
+        A = torch.randn((n, n, n), generator=g, dtype=torch.float32)
+        if even:   # A[n] == A[-n] about index floor(n/2): exercises the real-grid kernels
+            c = n // 2
+            idx = (2 * c - torch.arange(n)) % n
+            Af = A[idx][:, idx][:, :, idx]
+            A = 0.5 * (A + Af)
+            if n % 2 == 0:
+                A[0] = 0; A[:, 0] = 0; A[:, :, 0] = 0
+        rows = cols = 40     # 1,600 pixels: 8 x 16 lattice patches with ragged edges
+        u = (torch.arange(cols, dtype=torch.float64) - (cols - 1) / 2) / cols
+        v = (torch.arange(rows, dtype=torch.float64) - (rows - 1) / 2) / rows
+        vv, uu = torch.meshgrid(v, u, indexing="ij")
+        k = torch.stack([uu, vv, torch.ones_like(uu)], -1)
+        q = k / k.norm(dim=-1, keepdim=True) - torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64)
+        pix = (q * (0.9 * torch.pi / q.norm(dim=-1).max())).reshape(-1, 3).to(torch.float32)
+        quats = torch.randn((37, 4), generator=g, dtype=torch.float32)
+        ctx = SpfContext(n, eps=eps, device=device)
+        ctx.spf_set_detector_layout(1, rows, cols)
+        ctx.spf_prepare_model(A.to(dev))
+        assert bool(ctx.info.grid_is_real) == even
+        outs = []
+        for impl in (1, 0):
+            ctx.spf_set_option("slice_impl", impl)
+            outs.append(ctx.spf_slice(quats.to(dev), pix.to(dev), SPF_OUT_COMPLEX))
+            ctx.spf_check_fault()
+        err = float((outs[1] - outs[0]).abs().pow(2).sum().sqrt() / outs[0].abs().pow(2).sum().sqrt())
+        worst = max(worst, err)
+        # the two variants differ only in how the kernel weights are evaluated (polynomial fit vs exp/sqrt)
+        if not err <= 3e-6:
+            raise AssertionError("staged vs global gather: relative L2 %.3e (n=%d eps=%g)" % (err, n, eps))
+        ctx.close()
+    return "staged == global gather to %.1e" % worst
+
+
+def _check_match(device: int, cta_group: int) -> str:
+    import torch
+    from .binding import SpfContext
+    dev = torch.device("cuda", device)
+    g = torch.Generator(device="cpu"); g.manual_seed(5 + cta_group)
+    ctx = SpfContext(8, device=device)
+    ctx.spf_set_option("match_cta_group", cta_group)
+    worst = 0.0
+    for n_img, M, P, counts in ((300, 513, 2048, True), (130, 257, 200, False), (5, 40, 4100, True)):
+        S = torch.rand((M, P), generator=g) * torch.rand((M, 1), generator=g) * 3.0
+        pick = torch.randint(0, M, (n_img,), generator=g)
+        I = torch.poisson(S[pick], generator=g) if counts else S[pick] + 0.1 * torch.rand((n_img, P), generator=g)
+        mask = (torch.rand(P, generator=g) > 0.2).to(torch.uint8)
+        for mk in (None, mask):
+            dI, dS = I.to(dev).contiguous(), S.to(dev).contiguous()
+            dm = None if mk is None else mk.to(dev)
+            bi, bd = ctx.spf_match(dI, dS, dm)
+            ctx.spf_check_fault()
+            ri, rd, dist = ctx.spf_match_reference(dI, dS, dm)
+            torch.cuda.synchronize(dev)
+            rel = ((bd - rd).abs() / rd.clamp_min(1e-30)).max().item()
+            worst = max(worst, rel)
+            if not rel <= 1e-4:
+                raise AssertionError("cta_group %d: distance differs from the CUDA-core matcher by %.3e" % (cta_group, rel))
+            # argmin may differ only where the reference's own margin is within tolerance
+            d_at = dist.gather(1, bi.long().clamp(0, M - 1)[:, None])[:, 0]
+            bad = (bi != ri) & ((d_at - rd) > 1e-4 * rd)
+            if bool(bad.any()) or bool((bi < 0).any()) or bool((bi >= M).any()):
+                raise AssertionError("cta_group %d: argmin differs from the CUDA-core matcher" % cta_group)
+    ctx.close()
+    return "cta_group::%d == CUDA-core matcher, distances to %.1e" % (cta_group, worst)
+
+
+def run_variant(variant: str, device: int = 0) -> str:
+    if variant == "slice_staged":
+        return _check_slice_staged(device)
+    if variant == "match_cg1":
+        return _check_match(device, 1)
+    if variant == "match_cg2":
+        return _check_match(device, 2)
+    raise ValueError("unknown variant %r (one of %s)" % (variant, ", ".join(VARIANTS)))
+
+
+def check_in_child(variant: str, device: int = 0, timeout_s: float = 240.0) -> dict:
+    """Run one variant's check in a child process.  Returns {"ok", "status", "detail", "seconds"}."""
+    t0 = time.time()
+    cmd = [sys.executable, "-m", "paper_2109_05339_b200.selfcheck", variant, "--device", str(device)]
+    try:
+        p = subprocess.run(cmd, cwd=_ROOT, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, timeout=timeout_s)
+        status, out = p.returncode, p.stdout
+    except subprocess.TimeoutExpired as e:
+        status, out = -999, (e.stdout or "") if isinstance(e.stdout, str) else ""
+        out += "\n[selfcheck] timed out after %.0f s" % timeout_s
+    tail = [ln for ln in out.strip().splitlines() if ln.strip()][-3:]
+    return {"ok": status == 0, "status": status, "detail": " | ".join(tail)[-400:], "seconds": round(time.time() - t0, 1)}
+
+
+def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = None) -> dict:
+    """{variant: passed} for every variant, each checked once per process (cached)."""
+    out = {}
+    for v in VARIANTS:
+        key = (v, device)
+        if key not in _cache:
+            _cache[key] = check_in_child(v, device, timeout_s)
+            sys.stderr.write("[libspf selfcheck] %-12s %s (%s, %.1f s)\n" % (
+                v, "ok" if _cache[key]["ok"] else "FAILED status %s" % _cache[key]["status"], _cache[key]["detail"],
+                _cache[key]["seconds"]))
+        out[v] = _cache[key]["ok"]
+        if report is not None:
+            report[v] = _cache[key]
+    return out
+
+
+if __name__ == "__main__":
+    import argparse
+    ap = argparse.ArgumentParser(description=__doc__.split("\n")[0])
+    ap.add_argument("variant", choices=VARIANTS + ("all",))
+    ap.add_argument("--device", type=int, default=0)
+    a = ap.parse_args()
+    if a.variant == "all":
+        rep = {}
+        verified_variants(a.device, report=rep)
+        print(json.dumps(rep))
+        sys.exit(0 if all(r["ok"] for r in rep.values()) else 1)
+    try:
+        print("[selfcheck] %s: %s" % (a.variant, run_variant(a.variant, a.device)))
+    except Exception as e:   # disagreement, SPF_EFAULT from the watchdog, CUDA error
+        print("[selfcheck] %s FAILED: %s: %s" % (a.variant, type(e).__name__, e))
+        sys.exit(1)
