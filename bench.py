@@ -215,6 +215,9 @@ def run_spf(args, cfg):
     model, pix, mask, refs, truth, planted = host_inputs(cfg, rank)
     ctx = SpfContext(cfg.N, eps=cfg.eps, device=local)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    # kernel variants: the faster ones (TMA-staged gather, cta_group::2 GEMM) where their device self-check
+    # passes in a child process, else the library defaults (paper_2109_05339_b200/selfcheck.py)
+    variants = {"slice_staged": False, "match_cg2": False} if args.no_autotune else ctx.spf_autotune()
     info = ctx.info
     d_model = torch.from_numpy(model).to(dev)
     d_pix, d_refs = torch.from_numpy(pix).to(dev), torch.from_numpy(refs).to(dev)
@@ -246,6 +249,7 @@ def run_spf(args, cfg):
 
     for _ in range(max(args.warmup, 0)):
         step()
+    ctx.spf_check_fault()      # raises if any kernel's watchdog gave up: no number from a broken pipeline
     products = ctx.spf_last_match_products() if args.warmup > 0 else None
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
     k_ms = {"slice": [], "gemm": [], "match_prep": []}
@@ -264,6 +268,7 @@ def run_spf(args, cfg):
             k_ms["gemm"].append(ctx.spf_last_kernel_ms(1))
             k_ms["match_prep"].append(ctx.spf_last_kernel_ms(2))
         sync_all()
+    ctx.spf_check_fault()
     launches = ctx.spf_launch_count() - launches0
     if products is None:
         products = ctx.spf_last_match_products()
@@ -289,7 +294,11 @@ def run_spf(args, cfg):
             "data": "synthetic",
             "config": {"workload": cfg.name, "N": cfg.N, "n_fine": info.n_fine, "w": info.w, "P": cfg.P, "M": cfg.M,
                        "n_img_per_gpu": cfg.n_img, "eps": cfg.eps, "masked_frac": cfg.masked_frac,
-                       "grid_is_real": bool(info.grid_is_real), "parallelism": "images partitioned x%d, orientations replicated" % world,
+                       "grid_is_real": bool(info.grid_is_real),
+                       "kernel_variants": {"slice": "tma_staged" if variants.get("slice_staged") else "global_gather",
+                                           "match": "tcgen05 cta_group::%d" % (2 if variants.get("match_cg2") else 1),
+                                           "selfcheck": variants},
+                       "parallelism": "images partitioned x%d, orientations replicated" % world,
                        "l2": "inputs larger than L2 (slices %.2f GB, images %.2f GB per step; no flush needed)"
                              % (cfg.M * cfg.P * 4e-9, cfg.n_img * cfg.P * 4e-9)},
             "breakdown_ms": {"prepare_model": prepare_ms, "slice": slice_ms, "match": match_ms},
@@ -397,6 +406,7 @@ def main():
     ap.add_argument("--impl", default="spf", choices=["spf", "reference"])
     ap.add_argument("--config", default="paper_scale", choices=sorted(CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-autotune", action="store_true", help="library default kernel variants, no device self-check")
     args = ap.parse_args()
     if args.steps < 1:
         raise SystemExit("--steps must be >= 1")

@@ -148,10 +148,9 @@ def test_slice_general_model_widths_and_even_n(spf, N, eps):
     ctx = spf.SpfContext(N, eps=eps)
     ctx.spf_prepare_model(_dev(A))
     assert ctx.info.grid_is_real == 0
-    for impl in (0, 1):
-        ctx.spf_set_option("slice_impl", impl)
-        c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy()
-        assert _rel_l2(c, c_ref) <= max(SLICE_TOL, 10 * eps)
+    c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy()
+    ctx.spf_check_fault()
+    assert _rel_l2(c, c_ref) <= max(SLICE_TOL, 10 * eps)
 
 
 def test_slice_edge_cases(spf, tiny):
@@ -177,6 +176,7 @@ def test_slice_edge_cases(spf, tiny):
     edge = np.array([[np.pi, -np.pi, 0.0], [-np.pi, np.pi, np.pi], [3.14159, 3.14159, -3.14159]], np.float32)
     c = ctx.spf_slice(_dev(ident), _dev(edge), spf.SPF_OUT_COMPLEX).cpu().numpy()
     assert _rel_l2(c, orc.slice_points(model, ident, edge)) <= SLICE_TOL
+    ctx.spf_check_fault()
     with pytest.raises(spf.SpfError):
         spf.SpfContext(21, eps=0.0)
 
@@ -197,14 +197,21 @@ def test_slice_small_config_sampled(spf):
         ctx.spf_set_option("force_complex_grid", force_complex)
         c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX)
         got = c[torch.from_numpy(sm).cuda(), torch.from_numpy(sj).cuda()].cpu().numpy()
+        ctx.spf_check_fault()
         assert _rel_l2(got, ref) <= SLICE_TOL
 
 
 # --------------------------------------------------------------------------------- a6-a8: matching
 
-@pytest.mark.parametrize("cta_group", [2, 1])
-@pytest.mark.parametrize("n_img,M,P,masked", [(16, 64, 1024, False), (5, 300, 1000, True), (130, 257, 192, False), (300, 513, 2048, True)])
-def test_match_vs_oracle_ragged_sizes(spf, cta_group, n_img, M, P, masked):
+MATCH_SIZES = [(16, 64, 1024, False), (5, 300, 1000, True), (130, 257, 192, False), (300, 513, 2048, True)]
+
+
+@pytest.mark.parametrize("n_img,M,P,masked", MATCH_SIZES)
+def test_match_vs_oracle_ragged_sizes(spf, n_img, M, P, masked):
+    match_vs_oracle_ragged_sizes(spf, 1, n_img, M, P, masked)
+
+
+def match_vs_oracle_ragged_sizes(spf, cta_group, n_img, M, P, masked):
     rng = np.random.default_rng(n_img * 7 + M)
     S = (rng.random((M, P)) * rng.random((M, 1)) * 3).astype(np.float32)
     I = rng.poisson(S[rng.integers(0, M, n_img)]).astype(np.float32)
@@ -212,6 +219,7 @@ def test_match_vs_oracle_ragged_sizes(spf, cta_group, n_img, M, P, masked):
     ctx = spf.SpfContext(8)
     ctx.spf_set_option("match_cta_group", cta_group)
     bi, bd = ctx.spf_match(_dev(I), _dev(S), None if mask is None else _dev(mask))
+    ctx.spf_check_fault()
     _check_match(bi, bd, I, S, mask, "cg%d" % cta_group)
     # the independent CUDA-core reference agrees with the oracle too (and gives the full matrix)
     ri, rd, dist = ctx.spf_match_reference(_dev(I), _dev(S), None if mask is None else _dev(mask))
@@ -249,6 +257,7 @@ def test_match_planted_ties_and_general_values(spf):
     assert np.allclose(bdp.cpu().numpy(), bd.cpu().numpy(), rtol=1e-5)
     # empty image set is a no-op; M = 0 with images is an error
     assert ctx.spf_match(_dev(I[:0]), _dev(S))[0].shape == (0,)
+    ctx.spf_check_fault()
     with pytest.raises(spf.SpfError):
         ctx.spf_match(_dev(I), _dev(S[:0]))
 
@@ -271,6 +280,7 @@ def test_end_to_end_tiny_poisson(spf, tiny):
     assert np.all((bi == oi) | near)
     assert np.all(np.abs(bd - od) <= DIST_TOL * od)
     # host-buffer entry point gives the same answer
+    ctx.spf_check_fault()
     hi, hd, hs = ctx.spf_orientation_match_host(model, refs, pix, images, scale=alpha, want_slices=True)
     assert np.array_equal(hi, bi) and np.array_equal(hd, bd) and np.array_equal(hs, slices.cpu().numpy())
 
@@ -293,6 +303,7 @@ def test_end_to_end_small_subset(spf):
     bi, bd = ctx.spf_match(_dev(images), slices)
     oi, od, osd, _ = orc.match(images, alpha * c_ref.real)
     bi, bd = bi.cpu().numpy(), bd.cpu().numpy()
+    ctx.spf_check_fault()
     near = (osd - od) <= DIST_TOL * od
     assert np.all((bi == oi) | near) and np.all(np.abs(bd - od) <= DIST_TOL * od)
 
@@ -310,10 +321,13 @@ def test_paper_scale_sampled(spf):
     refs = random_quaternions(cfg.M, seed=2)
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    variants = ctx.spf_autotune()     # what bench.py does: the faster variants where the device self-check passes
+    print("paper-scale runs with", variants)
     ctx.spf_prepare_model(_dev(model))
     c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX)
     sm, sj = sample_pairs(cfg.M, cfg.P, 4096)
     got = c[torch.from_numpy(sm).cuda(), torch.from_numpy(sj).cuda()].cpu().numpy()
+    ctx.spf_check_fault()
     del c
     ref = orc.slice_points(model, refs, pix, sm, sj)
     assert _rel_l2(got, ref) <= SLICE_TOL
@@ -327,6 +341,7 @@ def test_paper_scale_sampled(spf):
     for s in range(0, cfg.n_img, 1000):
         images[s:s + 1000] = poisson_images(S[truth[s:s + 1000]], seed=4 + s)
     bi, bd = ctx.spf_match(images, S, _dev(mask))
+    ctx.spf_check_fault()
     rows = np.random.default_rng(6).choice(cfg.n_img, 24, replace=False)
     S_h = S.cpu().numpy()
     I_h = images[torch.from_numpy(rows).cuda()].cpu().numpy()

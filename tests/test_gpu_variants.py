@@ -1,0 +1,129 @@
+"""GPU parity of the faster kernel variants (-m gpu; collected after tests/test_gpu_parity.py).
+
+`slice_impl = 0` (TMA-staged shared-memory gather) and `match_cta_group = 2` (tcgen05 on CTA pairs)
+are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
+distances <= 1e-4, argmin exact outside near-ties.  Before a variant is launched in this process its
+device self-check (paper_2109_05339_b200/selfcheck.py) must have passed in a child process; if it did
+not, the test fails there, with the child's report, without launching the variant here.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from spf_inputs import CONFIGS, make_model, make_detector, random_quaternions, sample_pairs
+
+import test_gpu_parity as base
+from test_gpu_parity import spf, tiny, _dev, _rel_l2, SLICE_TOL, MATCH_SIZES  # noqa: F401  (fixtures)
+
+pytestmark = [pytest.mark.gpu, pytest.mark.timeout(1500)]
+
+
+@pytest.fixture(scope="module")
+def verified(spf):
+    from paper_2109_05339_b200 import selfcheck
+    report = {}
+    selfcheck.verified_variants(0, report=report)
+    return report
+
+
+def _require(verified, variant):
+    r = verified[variant]
+    if not r["ok"]:
+        pytest.fail("device self-check of %s did not pass (status %s): %s" % (variant, r["status"], r["detail"]))
+
+
+@pytest.mark.parametrize("variant", ["match_cg1", "slice_staged", "match_cg2"])
+def test_variant_selfcheck(verified, variant):
+    _require(verified, variant)
+
+
+# --------------------------------------------------------------------------------- staged slicing
+
+@pytest.mark.parametrize("force_complex,layout", [(0, True), (1, True), (0, False), (1, False)])
+def test_staged_slice_tiny_full(spf, tiny, verified, force_complex, layout):
+    _require(verified, "slice_staged")
+    base.slice_tiny_full(spf, tiny, 0, force_complex, layout)
+
+
+def test_staged_slice_equals_the_layout_free_result(spf, tiny, verified):
+    """Patch shape only changes which tile is staged, never the value: bit-identical outputs."""
+    _require(verified, "slice_staged")
+    cfg, model, pix, refs, _ = tiny
+    outs = []
+    for layout in ((1, 32, 32), (4, 16, 16), (0, 0, 0)):
+        ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+        ctx.spf_set_option("slice_impl", 0)
+        ctx.spf_set_detector_layout(*layout)
+        ctx.spf_prepare_model(_dev(model))
+        outs.append(ctx.spf_slice(_dev(refs[:8]), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy())
+        ctx.spf_check_fault()
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
+@pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9)])
+def test_staged_slice_general_model(spf, verified, N, eps):
+    """Non-even model (complex fine grid), even and odd N, w = 7 and w = 10."""
+    _require(verified, "slice_staged")
+    rng = np.random.default_rng(4)
+    A = rng.standard_normal((N, N, N)).astype(np.float32)
+    pix = make_detector(1, 16)
+    refs = random_quaternions(9, seed=31)
+    c_ref = orc.slice_points(A, refs, pix)
+    ctx = spf.SpfContext(N, eps=eps)
+    ctx.spf_set_option("slice_impl", 0)
+    ctx.spf_set_detector_layout(1, 16, 16)
+    ctx.spf_prepare_model(_dev(A))
+    c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy()
+    ctx.spf_check_fault()
+    assert _rel_l2(c, c_ref) <= max(SLICE_TOL, 10 * eps)
+
+
+def test_staged_slice_small_config_sampled(spf, verified):
+    """Small (configs[1]) through the staged kernel, real and complex grid, 4,096 oracle samples."""
+    _require(verified, "slice_staged")
+    cfg = CONFIGS["small"]
+    model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(cfg.M, seed=2)
+    ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+    ctx.spf_set_option("slice_impl", 0)
+    ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    ctx.spf_prepare_model(_dev(model))
+    sm, sj = sample_pairs(cfg.M, cfg.P, 4096)
+    ref = orc.slice_points(model, refs, pix, sm, sj)
+    for force_complex in (0, 1):
+        ctx.spf_set_option("force_complex_grid", force_complex)
+        c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX)
+        got = c[torch.from_numpy(sm).cuda(), torch.from_numpy(sj).cuda()].cpu().numpy()
+        ctx.spf_check_fault()
+        assert _rel_l2(got, ref) <= SLICE_TOL
+
+
+# --------------------------------------------------------------------------------- CTA-pair matching
+
+@pytest.mark.parametrize("n_img,M,P,masked", MATCH_SIZES)
+def test_cta_pair_match_vs_oracle_ragged_sizes(spf, verified, n_img, M, P, masked):
+    _require(verified, "match_cg2")
+    base.match_vs_oracle_ragged_sizes(spf, 2, n_img, M, P, masked)
+
+
+def test_cta_pair_and_single_cta_agree_on_counts(spf, verified):
+    """Photon-count images are exact in one fp16 plane (2 products per K step) and both variants add
+    the same products in the same K order into fp32 accumulators: distances agree to fp32 round-off."""
+    _require(verified, "match_cg2")
+    rng = np.random.default_rng(23)
+    M, P, n_img = 700, 3000, 260
+    S = (rng.random((M, P)) * 2).astype(np.float32)
+    I = rng.poisson(S[rng.integers(0, M, n_img)]).astype(np.float32)
+    ctx = spf.SpfContext(8)
+    res = []
+    for cg in (1, 2):
+        ctx.spf_set_option("match_cta_group", cg)
+        bi, bd = ctx.spf_match(_dev(I), _dev(S))
+        ctx.spf_check_fault()
+        assert ctx.spf_last_match_products() == 2
+        res.append((bi.cpu().numpy(), bd.cpu().numpy()))
+    assert np.allclose(res[0][1], res[1][1], rtol=2e-6)
+    for bi, bd in res:
+        base._check_match(torch.from_numpy(bi), torch.from_numpy(bd), I, S, None, "counts")
