@@ -18,28 +18,32 @@
 
 #include "ptx_sm100.cuh"
 #include "spf_internal.cuh"
+#include "spf_match_math.cuh"
 
 namespace {
 
-constexpr int BK = 64;                            // fp16 elements per K block: 128 bytes, one swizzle row
-constexpr int BN = 256;                           // slices per tile (UMMA N)
-constexpr int TILE_ROWS = 128;                    // image rows per CTA (UMMA M = 128 * CG)
-constexpr int A_TILE_BYTES = TILE_ROWS * BK * 2;  // 16 KB
-constexpr int GEMM_THREADS = 192;                 // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
+using spfmm::BK;         // 64 fp16 per K block: 128 bytes, one swizzle row
+using spfmm::BN;         // 256 slices per tile (UMMA N)
+using spfmm::TILE_ROWS;  // 128 image rows per CTA (UMMA M = 128 * CG)
+using spfmm::A_TILE_BYTES;
+constexpr int EPI_WARPS = 8;                      // two per TMEM lane quadrant, each takes one half of the tile's columns
+constexpr int GEMM_THREADS = 64 + 32 * EPI_WARPS; // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-9 epilogue
+constexpr int EPI_COLS = BN / (EPI_WARPS / 4);    // 128 accumulator registers per epilogue thread
+using spfmm::CHUNK_KB;
 constexpr int ACC_STAGES = 2;
 constexpr int TMEM_COLS = ACC_STAGES * BN;        // 512: all of TMEM, one CTA per SM
-constexpr size_t SMEM_AUX = 6144;                 // 1 KB barriers, tmem pointer, abort word; 4 KB per-warp ||S||^2 tiles
-constexpr size_t SMEM_BUDGET = 227 * 1024;
+constexpr size_t SMEM_AUX = spfmm::SMEM_AUX;
 
 template <int CG, int NI>
 struct GemmCfg {
-    static constexpr int B_ROWS = BN / CG;                      // slice rows this CTA stages
-    static constexpr int B_TILE_BYTES = B_ROWS * BK * 2;
-    static constexpr int STAGE_BYTES = NI * A_TILE_BYTES + 2 * B_TILE_BYTES;
-    static constexpr int STAGES_RAW = (int)((SMEM_BUDGET - SMEM_AUX - 1024) / STAGE_BYTES);
-    static constexpr int STAGES = STAGES_RAW > 6 ? 6 : STAGES_RAW;
+    static constexpr int B_ROWS = spfmm::b_rows(CG);            // slice rows this CTA stages
+    static constexpr int B_TILE_BYTES = spfmm::b_tile_bytes(CG);
+    static constexpr int STAGE_BYTES = spfmm::stage_bytes(CG, NI);
+    static constexpr int STAGES = spfmm::stages(CG, NI);
     static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + SMEM_AUX + 1024;
+    static constexpr int OFF_A1 = spfmm::off_a(1), OFF_B0 = spfmm::off_b(CG, NI, 0), OFF_B1 = spfmm::off_b(CG, NI, 1);
     static_assert(STAGES >= 2, "need at least a double buffer");
+    static_assert(SMEM_BYTES <= (size_t)spfmm::SMEM_BUDGET, "shared memory budget");
 };
 
 struct MatchArgs {
@@ -89,16 +93,6 @@ __global__ void k_absmax(const float *__restrict__ x, int64_t rows, int64_t P, c
     if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
 }
 
-__device__ __forceinline__ int scale_exponent(uint32_t absmax_bits) {
-    // 2^e * max in [2^14, 2^15): fp16 holds it with 11 significant bits, products stay far from overflow
-    float mx = __uint_as_float(absmax_bits);
-    if (!(mx > 0.0f) || isinf(mx) || isnan(mx)) return 0;
-    int k;
-    frexpf(mx, &k);  // mx = f * 2^k, f in [0.5, 1)
-    int e = 15 - k;
-    return max(-100, min(100, e));
-}
-
 // One block per row: x * 2^e = h1 + h2 as two fp16 planes (zero in masked pixels and in the K padding),
 // ||x||^2 over unmasked pixels accumulated in fp64, and (images) the running-argmin key reset.
 // which = 0: images (sets scal[2] when some residual is non-zero, resets keys), 1: slices.
@@ -107,7 +101,7 @@ __global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int6
                                                int64_t rows, __half *__restrict__ planes, float *__restrict__ norms,
                                                unsigned long long *__restrict__ keys) {
     const int64_t row = blockIdx.x;
-    const int e = scale_exponent(scal[which]);
+    const int e = spfmm::scale_exponent(scal[which]);
     const float sc = ldexpf(1.0f, e);
     const float *xr = x + row * P;
     __half *h1 = planes + row * Ppad, *h2 = planes + (rows + row) * Ppad;
@@ -117,13 +111,10 @@ __global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int6
         float v = 0.0f;
         if (c < P && (!mask || mask[c])) v = xr[c];
         acc += (double)v * (double)v;
-        float vs = v * sc;
-        __half a = __float2half_rn(vs);
-        float r = vs - __half2float(a);
-        __half b = __float2half_rn(r);
-        inexact |= (r != 0.0f);
-        h1[c] = a;
-        h2[c] = b;
+        uint16_t a, b;
+        inexact |= spfmm::split_fp16(v, sc, a, b);
+        h1[c] = __ushort_as_half(a);
+        h2[c] = __ushort_as_half(b);
     }
     __shared__ double red[8];
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -142,21 +133,13 @@ __global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int6
     }
 }
 
-__device__ __forceinline__ uint32_t orderable(float d) {
-    uint32_t u = __float_as_uint(d);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-__device__ __forceinline__ float unorderable(uint32_t u) {
-    return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
-}
-
 __global__ void k_match_finalize(const unsigned long long *__restrict__ keys, int64_t n_img, int32_t *__restrict__ best_idx,
                                  float *__restrict__ best_dist) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= n_img) return;
     unsigned long long k = keys[i];
     best_idx[i] = (int32_t)(uint32_t)(k & 0xffffffffull);  // -1 if no finite distance was seen
-    best_dist[i] = (k == ~0ull) ? __uint_as_float(0x7fc00000u) : unorderable((uint32_t)(k >> 32));
+    best_dist[i] = (k == ~0ull) ? __uint_as_float(0x7fc00000u) : spfmm::unorderable((uint32_t)(k >> 32));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -179,7 +162,7 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     const uint32_t bar_full = aux, bar_empty = aux + 8 * ST, bar_tfull = aux + 16 * ST, bar_tempty = bar_tfull + 8 * ACC_STAGES;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(aux_p + 16 * ST + 16 * ACC_STAGES);
     volatile uint32_t *abort_w = tmem_slot + 1;              // raised by the first wait that gives up
-    float *nsbuf = reinterpret_cast<float *>(aux_p + 1024);  // [4 epilogue warps][BN]
+    float *nsbuf = reinterpret_cast<float *>(aux_p + 1024);  // [EPI_WARPS][EPI_COLS]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
@@ -192,7 +175,7 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
         ptx::prefetch_tensormap(&mapA0); ptx::prefetch_tensormap(&mapB0); ptx::prefetch_tensormap(&mapB1);
         if (NI == 2) ptx::prefetch_tensormap(&mapA1);
         for (int s = 0; s < ST; ++s) { ptx::mbar_init(bar_full + 8 * s, 1); ptx::mbar_init(bar_empty + 8 * s, 1); }
-        for (int s = 0; s < ACC_STAGES; ++s) { ptx::mbar_init(bar_tfull + 8 * s, 1); ptx::mbar_init(bar_tempty + 8 * s, 4 * CG); }
+        for (int s = 0; s < ACC_STAGES; ++s) { ptx::mbar_init(bar_tfull + 8 * s, 1); ptx::mbar_init(bar_tempty + 8 * s, EPI_WARPS * CG); }
         ptx::fence_mbar_init();
     }
     if (warp == 1) ptx::tmem_alloc<CG>(ptx::smem_u32(tmem_slot), TMEM_COLS);
@@ -201,16 +184,7 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    auto tile_coords = [&](int t, int &ib, int &mb) {
-        // groups of 8 image blocks, slice tiles fastest across groups' members: concurrently
-        // running tiles share operand rows in L2
-        const int G = 8;
-        const int per_group = G * a.n_mb;
-        const int g = t / per_group, r = t - g * per_group;
-        const int gsz = min(G, a.n_ib - g * G);
-        ib = g * G + r % gsz;
-        mb = r / gsz;
-    };
+    auto tile_coords = [&](int t, int &ib, int &mb) { spfmm::tile_coords(t, a.n_ib, a.n_mb, ib, mb); };
 
     // a wait that gave up: note where (first writer wins is not needed -- any one record will do)
     auto give_up = [&](uint32_t role, int t) {
@@ -239,14 +213,14 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
                     const int kc = kb * BK;
                     if (CG == 1) {
                         ptx::tma_load_2d(st, &mapA0, kc, rowA, fb);
-                        if (NI == 2) ptx::tma_load_2d(st + A_TILE_BYTES, &mapA1, kc, rowA, fb);
-                        ptx::tma_load_2d(st + NI * A_TILE_BYTES, &mapB0, kc, rowB, fb);
-                        ptx::tma_load_2d(st + NI * A_TILE_BYTES + Cfg::B_TILE_BYTES, &mapB1, kc, rowB, fb);
+                        if (NI == 2) ptx::tma_load_2d(st + Cfg::OFF_A1, &mapA1, kc, rowA, fb);
+                        ptx::tma_load_2d(st + Cfg::OFF_B0, &mapB0, kc, rowB, fb);
+                        ptx::tma_load_2d(st + Cfg::OFF_B1, &mapB1, kc, rowB, fb);
                     } else {
                         ptx::tma_load_2d_2sm(st, &mapA0, kc, rowA, fb);
-                        if (NI == 2) ptx::tma_load_2d_2sm(st + A_TILE_BYTES, &mapA1, kc, rowA, fb);
-                        ptx::tma_load_2d_2sm(st + NI * A_TILE_BYTES, &mapB0, kc, rowB, fb);
-                        ptx::tma_load_2d_2sm(st + NI * A_TILE_BYTES + Cfg::B_TILE_BYTES, &mapB1, kc, rowB, fb);
+                        if (NI == 2) ptx::tma_load_2d_2sm(st + Cfg::OFF_A1, &mapA1, kc, rowA, fb);
+                        ptx::tma_load_2d_2sm(st + Cfg::OFF_B0, &mapB0, kc, rowB, fb);
+                        ptx::tma_load_2d_2sm(st + Cfg::OFF_B1, &mapB1, kc, rowB, fb);
                     }
                 }
                 __syncwarp();
@@ -260,72 +234,90 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
             int s = 0; uint32_t ph = 0; int as = 0; uint32_t aph = 0;
             bool alive = true;
             for (int t = cluster_id; alive && t < n_tiles; t += n_clusters) {
-                // epilogue has drained this accumulator stage
-                if (!ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u, abort_w)) { give_up(1, t); break; }
-                ptx::tc_fence_after();
-                const uint32_t tacc = tmem_base + (uint32_t)(as * BN);
-                for (int kb = 0; kb < a.kblocks; ++kb) {
-                    if (!ptx::mbar_wait(bar_full + 8 * s, ph, abort_w)) { give_up(2, t); alive = false; break; }
+                // K runs in chunks of CHUNK_KB blocks; each chunk starts on a cleared accumulator stage
+                // and is handed to the epilogue warps, which keep the running sum (spf_match_math.cuh)
+                for (int kb0 = 0; alive && kb0 < a.kblocks; kb0 += CHUNK_KB) {
+                    // epilogue has drained this accumulator stage
+                    if (!ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u, abort_w)) { give_up(1, t); alive = false; break; }
                     ptx::tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
-                        const uint64_t dA0 = ptx::umma_desc_sw128(st);
-                        const uint64_t dA1 = ptx::umma_desc_sw128(st + A_TILE_BYTES);
-                        const uint64_t dB0 = ptx::umma_desc_sw128(st + NI * A_TILE_BYTES);
-                        const uint64_t dB1 = ptx::umma_desc_sw128(st + NI * A_TILE_BYTES + Cfg::B_TILE_BYTES);
+                    const uint32_t tacc = tmem_base + (uint32_t)(as * BN);
+                    const int kend = min(kb0 + CHUNK_KB, a.kblocks);
+                    for (int kb = kb0; kb < kend; ++kb) {
+                        if (!ptx::mbar_wait(bar_full + 8 * s, ph, abort_w)) { give_up(2, t); alive = false; break; }
+                        ptx::tc_fence_after();
+                        if (lane == 0) {
+                            const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
+                            const uint64_t dA0 = ptx::umma_desc_sw128(st);
+                            const uint64_t dA1 = ptx::umma_desc_sw128(st + Cfg::OFF_A1);
+                            const uint64_t dB0 = ptx::umma_desc_sw128(st + Cfg::OFF_B0);
+                            const uint64_t dB1 = ptx::umma_desc_sw128(st + Cfg::OFF_B1);
 #pragma unroll
-                        for (int k4 = 0; k4 < BK / 16; ++k4) {  // 16 fp16 = 32 bytes per UMMA K step: +2 in the address field
-                            const uint64_t ko = (uint64_t)(k4 * 2);
-                            ptx::umma_f16<CG>(tacc, dA0 + ko, dB0 + ko, idesc, (uint32_t)((kb | k4) != 0));
-                            ptx::umma_f16<CG>(tacc, dA0 + ko, dB1 + ko, idesc, 1u);
-                            if (NI == 2) ptx::umma_f16<CG>(tacc, dA1 + ko, dB0 + ko, idesc, 1u);
+                            for (int k4 = 0; k4 < BK / 16; ++k4) {  // 16 fp16 = 32 bytes per UMMA K step: +2 in the address field
+                                const uint64_t ko = (uint64_t)(k4 * 2);
+                                ptx::umma_f16<CG>(tacc, dA0 + ko, dB0 + ko, idesc, (uint32_t)(kb != kb0 || k4 != 0));
+                                ptx::umma_f16<CG>(tacc, dA0 + ko, dB1 + ko, idesc, 1u);
+                                if (NI == 2) ptx::umma_f16<CG>(tacc, dA1 + ko, dB0 + ko, idesc, 1u);
+                            }
+                            ptx::umma_commit<CG>(bar_empty + 8 * s);                       // smem slot free when these MMAs retire
+                            if (kb == kend - 1) ptx::umma_commit<CG>(bar_tfull + 8 * as);  // chunk complete
                         }
-                        ptx::umma_commit<CG>(bar_empty + 8 * s);                              // smem slot free when these MMAs retire
-                        if (kb == a.kblocks - 1) ptx::umma_commit<CG>(bar_tfull + 8 * as);   // accumulator complete
+                        __syncwarp();
+                        if (++s == ST) { s = 0; ph ^= 1u; }
                     }
-                    __syncwarp();
-                    if (++s == ST) { s = 0; ph ^= 1u; }
+                    if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
                 }
-                if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
             }
         }
     } else {
-        // ===================== epilogue: TMEM -> registers -> norm add + running argmin =====================
-        // Each warp works alone (its own TMEM lane quadrant, its own copy of the tile's ||S||^2), so
-        // the four warps never wait for one another.
-        const int q = warp & 3;                 // TMEM lane quadrant this warp may read
-        float *nsb = nsbuf + (warp - 2) * BN;
-        const float neg2sc = ldexpf(-2.0f, -((int)a.scal[4] + (int)a.scal[5]));
+        // ===================== epilogue: TMEM chunks -> fp32 registers -> norm add + running argmin =====================
+        // Warp (warp - 2) reads TMEM lane quadrant warp % 4 (the only one the hardware lets it read) and
+        // the column half (warp - 2) / 4 of the tile: thread = one image row x EPI_COLS slices, whose
+        // cross terms it sums chunk by chunk in registers (round to nearest).  Each warp works alone --
+        // its own lanes, its own copy of its ||S||^2 values -- so epilogue warps never wait for one another.
+        const int ew = warp - 2;
+        const int q = warp & 3;                 // TMEM lane quadrant
+        const int col0 = (ew >> 2) * EPI_COLS;  // first tile column of this warp
+        float *nsb = nsbuf + ew * EPI_COLS;
+        const float neg2sc = spfmm::cross_scale((int)a.scal[4], (int)a.scal[5]);
         int as = 0; uint32_t aph = 0;
-        for (int t = cluster_id; t < n_tiles; t += n_clusters) {
+        bool alive = true;
+        for (int t = cluster_id; alive && t < n_tiles; t += n_clusters) {
             int ib, mb; tile_coords(t, ib, mb);
-            const int64_t m0 = (int64_t)mb * BN;
+            const int64_t m0 = (int64_t)mb * BN + col0;
             __syncwarp();
-            for (int k = lane; k < BN; k += 32) nsb[k] = (m0 + k < a.M) ? a.nS[m0 + k] : INFINITY;
+            for (int k = lane; k < EPI_COLS; k += 32) nsb[k] = (m0 + k < a.M) ? a.nS[m0 + k] : INFINITY;
             __syncwarp();
             const int64_t i = (int64_t)ib * (TILE_ROWS * CG) + (int64_t)rank * TILE_ROWS + q * 32 + lane;
             const float nIv = (i < a.n_img) ? a.nI[i] : 0.0f;
-            if (!ptx::mbar_wait(bar_tfull + 8 * as, aph, abort_w)) { give_up(3, t); break; }
-            ptx::tc_fence_after();
-            float best = INFINITY; uint32_t bm = 0xffffffffu;
-            const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * BN);
-#pragma unroll 1
-            for (int c = 0; c < BN / 32; ++c) {
-                uint32_t r[32];
-                ptx::tmem_ld_32x32(trow + c * 32, r);
-                ptx::tmem_ld_wait();
+            float acc[EPI_COLS];
 #pragma unroll
-                for (int k = 0; k < 32; ++k) {
-                    const float d = nIv + fmaf(neg2sc, __uint_as_float(r[k]), nsb[c * 32 + k]);
-                    if (d < best) { best = d; bm = (uint32_t)(m0 + c * 32 + k); }
+            for (int k = 0; k < EPI_COLS; ++k) acc[k] = 0.0f;
+            for (int kb0 = 0; kb0 < a.kblocks; kb0 += CHUNK_KB) {
+                if (!ptx::mbar_wait(bar_tfull + 8 * as, aph, abort_w)) { give_up(3, t); alive = false; break; }
+                ptx::tc_fence_after();
+                const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * BN + col0);
+#pragma unroll
+                for (int c = 0; c < EPI_COLS / 32; ++c) {
+                    uint32_t r[32];
+                    ptx::tmem_ld_32x32(trow + c * 32, r);
+                    ptx::tmem_ld_wait();
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) acc[c * 32 + k] += __uint_as_float(r[k]);
                 }
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) { if (CG == 2) ptx::mbar_arrive_cluster(bar_tempty + 8 * as, 0); else ptx::mbar_arrive(bar_tempty + 8 * as); }
+                if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
             }
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) { if (CG == 2) ptx::mbar_arrive_cluster(bar_tempty + 8 * as, 0); else ptx::mbar_arrive(bar_tempty + 8 * as); }
+            if (!alive) break;
+            float best = INFINITY; uint32_t bm = 0xffffffffu;
+#pragma unroll
+            for (int k = 0; k < EPI_COLS; ++k) {
+                const float d = spfmm::distance(nIv, nsb[k], neg2sc, acc[k]);
+                if (d < best) { best = d; bm = (uint32_t)(m0 + k); }
+            }
             if (i < a.n_img && bm != 0xffffffffu)
-                atomicMin(&a.keys[i], ((unsigned long long)orderable(best) << 32) | bm);
-            if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
+                atomicMin(&a.keys[i], spfmm::pack_key(best, bm));
         }
     }
 
