@@ -215,9 +215,10 @@ def run_spf(args, cfg):
     model, pix, mask, refs, truth, planted = host_inputs(cfg, rank)
     ctx = SpfContext(cfg.N, eps=cfg.eps, device=local)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    # kernel variants: the faster ones (TMA-staged gather, cta_group::2 GEMM) where their device self-check
+    # kernel variants: the faster ones (TMA-staged gather -- the fastest verified form --, cta_group::2 GEMM) where their device self-check
     # passes in a child process, else the library defaults (paper_2109_05339_b200/selfcheck.py)
-    variants = {"slice_staged": False, "match_cg2": False} if args.no_autotune else ctx.spf_autotune()
+    variants = ({"slice_staged": False, "slice_coop": False, "match_cg2": False, "slice_impl": 1, "match_cta_group": 1}
+                if args.no_autotune else ctx.spf_autotune())
     info = ctx.info
     d_model = torch.from_numpy(model).to(dev)
     d_pix, d_refs = torch.from_numpy(pix).to(dev), torch.from_numpy(refs).to(dev)
@@ -295,8 +296,9 @@ def run_spf(args, cfg):
             "config": {"workload": cfg.name, "N": cfg.N, "n_fine": info.n_fine, "w": info.w, "P": cfg.P, "M": cfg.M,
                        "n_img_per_gpu": cfg.n_img, "eps": cfg.eps, "masked_frac": cfg.masked_frac,
                        "grid_is_real": bool(info.grid_is_real),
-                       "kernel_variants": {"slice": "tma_staged" if variants.get("slice_staged") else "global_gather",
-                                           "match": "tcgen05 cta_group::%d" % (2 if variants.get("match_cg2") else 1),
+                       "kernel_variants": {"slice": {0: "tma_staged, thread per point", 1: "global_gather, thread per point",
+                                                     2: "tma_staged, warp per point"}[variants["slice_impl"]],
+                                           "match": "tcgen05 cta_group::%d" % variants["match_cta_group"],
                                            "selfcheck": variants},
                        "parallelism": "images partitioned x%d, orientations replicated" % world,
                        "l2": "inputs larger than L2 (slices %.2f GB, images %.2f GB per step; no flush needed)"

@@ -14,12 +14,7 @@
 
 #define SPF_MAX_W 16
 
-// One TMA tensor map per (box_z, box_y) combination used by the slicing kernel to stage a
-// fine-grid tile: boxes are {SPF_BOX_MIN, +4, ..., SPF_BOX_MAX} cells along z and y, one x-plane deep.
-#define SPF_BOX_MIN 8
-#define SPF_BOX_MAX 40
-#define SPF_BOX_STEP 4
-#define SPF_BOX_N ((SPF_BOX_MAX - SPF_BOX_MIN) / SPF_BOX_STEP + 1)  // 9
+#include "spf_slice_math.cuh"  // SPF_BOX_*: the menu of TMA box sizes (one tensor map per (by, bz) pair)
 
 struct SliceMaps {
     CUtensorMap m[SPF_BOX_N * SPF_BOX_N];  // [iy * SPF_BOX_N + iz]

@@ -17,6 +17,7 @@
 #include <limits.h>
 #include <math.h>
 
+#include <type_traits>
 #include <vector>
 
 #include "ptx_sm100.cuh"
@@ -48,9 +49,25 @@ __device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t
     else reinterpret_cast<float *>(a.out)[m * a.P + j] = a.scale * c.x;
 }
 
+// Kernel variants (option "slice_impl"):
+//   IMPL_GLOBAL  1  one thread per point, w^3 loads straight from the grid in global memory (L1/L2)
+//   IMPL_STAGED  0  tile staged by TMA, one thread per point gathers from shared memory
+//   IMPL_COOP    2  tile staged by TMA, a WARP gathers each point: lane (h, k) reads rows h, h + 4 and
+//                   cell k of the point's 8 x 8 window in every x-plane -- 32 consecutive-bank words per
+//                   load, no bank conflicts (spf_slice_math.cuh) -- and a shuffle tree adds the 32
+//                   partial sums.  One thread per point has its lanes scattered over the tile (the
+//                   rotated lattice is generic), which costs a conflict degree of ~3.5 per load
+//                   (DESIGN.md section 5); the warp-per-point form needs 14 conflict-free loads + 4
+//                   weight loads per point instead of 343 loads / 32 lanes x 3.5.
+enum { IMPL_STAGED = 0, IMPL_GLOBAL = 1, IMPL_COOP = 2 };
+#define SPF_COOP_WTS_BYTES (SPF_PATCH * SPF_COOP_STRIDE * 4)   // 14,336 = 112 x 128
+
 // W = 0: runtime kernel width (any w <= SPF_MAX_W), else compile-time.
-template <int W, bool REAL, int OUTK, bool STAGED>
-__global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __grid_constant__ SliceArgs a) {
+template <int W, bool REAL, int OUTK, int IMPL>
+__global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slice(const __grid_constant__ SliceArgs a) {
+    constexpr bool STAGED = (IMPL != IMPL_GLOBAL);
+    constexpr bool COOP = (IMPL == IMPL_COOP);
+    static_assert(!COOP || (W >= 2 && W <= 8), "the cooperative gather reads an 8 x 8 window per x-plane");
     constexpr int WMAX = W ? W : SPF_MAX_W;
     constexpr int E = REAL ? 1 : 2;            // floats per cell
     constexpr int CELL = 4 * E;                // bytes per cell
@@ -63,7 +80,9 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
     __shared__ int s_lo[3], s_hi[3];
     __shared__ __align__(8) unsigned long long s_bar;
     __shared__ uint32_t s_abort;
-    extern __shared__ __align__(128) uint8_t s_tile[];
+    extern __shared__ __align__(128) uint8_t s_dyn[];
+    // cooperative variant: the first SPF_COOP_WTS_BYTES of dynamic shared memory hold the points' weights
+    uint8_t *s_tile = s_dyn + (COOP ? SPF_COOP_WTS_BYTES : 0);
 
     if (tid == 0) {
         spfm::quat_to_R(a.quats + 4 * m, sR);
@@ -97,17 +116,17 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
         }
         __syncthreads();
         lox = s_lo[0]; loy = s_lo[1]; loz = s_lo[2];
-        const int Lx = s_hi[0] - lox + w, Ly = s_hi[1] - loy + w, Lz = s_hi[2] - loz + w;
-        const int by = max(SPF_BOX_MIN, (Ly + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP);
-        bz = max(SPF_BOX_MIN, (Lz + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP);
-        // x-plane pitch: TMA shared-memory destinations are kept 128-byte aligned
-        S1 = (by * bz + (128 / CELL) - 1) / (128 / CELL) * (128 / CELL);
-        staged = (by <= SPF_BOX_MAX) && (bz <= SPF_BOX_MAX) && ((uint32_t)(Lx * S1 * CELL) <= a.cap_bytes);
+        // a patch with no pixel at all (cannot happen with the tables build_patches makes) has lo > hi: not staged
+        const bool any = s_hi[0] >= lox;
+        const int Lx = any ? s_hi[0] - lox + w : 0, Ly = any ? s_hi[1] - loy + w : 0, Lz = any ? s_hi[2] - loz + w : 0;
+        const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, a.cap_bytes, COOP);
+        bz = g.bz; S1 = g.S1;
+        staged = g.ok;
         if (staged && tid < 32) {
             const uint32_t bar = ptx::smem_u32(&s_bar);
-            if (tid == 0) ptx::mbar_expect_tx(bar, (uint32_t)(Lx * by * bz * CELL));
+            if (tid == 0) ptx::mbar_expect_tx(bar, (uint32_t)(Lx * g.by * bz * CELL));
             __syncwarp();
-            const CUtensorMap *map = &a.maps.m[((by - SPF_BOX_MIN) / SPF_BOX_STEP) * SPF_BOX_N + (bz - SPF_BOX_MIN) / SPF_BOX_STEP];
+            const CUtensorMap *map = &a.maps.m[spfm::tile_map_index(g.by, bz)];
             const uint32_t dst = ptx::smem_u32(s_tile);
             for (int x = tid; x < Lx; x += 32)
                 ptx::tma_load_3d(dst + (uint32_t)(x * S1 * CELL), map, loz * E, loy, lox + x, bar);
@@ -125,18 +144,53 @@ __global__ void __launch_bounds__(SPF_PATCH, STAGED ? 3 : 4) k_slice(const __gri
     }
 
     spfm::c2 c;
+    c.x = c.y = 0.0f;
     if (STAGED && staged) {
+        if (COOP) {
+            // every lane parks its point's weights where its warp will read them back
+            float pk[24];
+            spfm::coop_pack_weights<WMAX>(pk, w, wx, wy, wz);
+            float4 *dst4 = reinterpret_cast<float4 *>(reinterpret_cast<float *>(s_dyn) + tid * SPF_COOP_STRIDE);
+#pragma unroll
+            for (int v = 0; v < 6; ++v) dst4[v] = make_float4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
+            __syncwarp();
+        }
         if (!ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort)) {
             if (tid == 0) {
-                a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)patch; a.fault[3] = (uint32_t)(W * 10 + (REAL ? 1 : 0));
+                a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)patch; a.fault[3] = (uint32_t)(W * 10 + (REAL ? 1 : 0) + 100 * IMPL);
                 a.fault[0] = SPF_FAULT_SLICE;
                 __threadfence_system();
             }
             return;
         }
-        if (!active) return;
-        const float *base = reinterpret_cast<const float *>(s_tile) + (size_t)((px - lox) * S1 + (py - loy) * bz + (pz - loz)) * E;
-        c = spfm::gather<WMAX, REAL>(base, S1, bz, w, wx, wy, wz);
+        const float *tile = reinterpret_cast<const float *>(s_tile);
+        const int cell = active ? (px - lox) * S1 + (py - loy) * bz + (pz - loz) : -1;
+        if (COOP) {
+            const int lane = tid & 31, h = lane >> 3, k = lane & 7;
+            const float *wts_warp = reinterpret_cast<const float *>(s_dyn) + (tid & ~31) * SPF_COOP_STRIDE;
+            // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates
+            auto sweep = [&](auto bz_tag) {
+                constexpr int BZ = decltype(bz_tag)::value;
+                for (int p = 0; p < 32; ++p) {
+                    const int cell_p = __shfl_sync(0xffffffffu, cell, p);
+                    if (cell_p < 0) continue;    // warp-uniform: an empty slot of a ragged patch
+                    spfm::c2 part = spfm::gather_coop_lane<REAL, BZ>(tile, cell_p, S1, bz, w, wts_warp + p * SPF_COOP_STRIDE, h, k);
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        part.x += __shfl_xor_sync(0xffffffffu, part.x, o);
+                        if (!REAL) part.y += __shfl_xor_sync(0xffffffffu, part.y, o);
+                    }
+                    if (lane == p) c = part;
+                }
+            };
+            if (bz == 24) sweep(std::integral_constant<int, 24>{});
+            else if (bz == 8) sweep(std::integral_constant<int, 8>{});
+            else sweep(std::integral_constant<int, 40>{});
+            if (!active) return;
+        } else {
+            if (!active) return;
+            c = spfm::gather<WMAX, REAL>(tile + (size_t)cell * E, S1, bz, w, wx, wy, wz);
+        }
     } else {
         if (!active) return;
         const float *base = a.grid + ((size_t)((size_t)px * a.np + py) * a.sz + pz) * E;
@@ -178,32 +232,39 @@ int build_patches(spf_ctx *ctx, int64_t P) {
     return SPF_OK;
 }
 
-template <int W, bool REAL, int OUTK, bool STAGED>
-int launch_slice(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, cudaStream_t st) {
-    auto kern = k_slice<W, REAL, OUTK, STAGED>;
-    if (STAGED) SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+template <int W, bool REAL, int OUTK, int IMPL>
+int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
+    auto kern = k_slice<W, REAL, OUTK, IMPL>;
+    // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid
+    uint32_t smem = 0;
+    args.cap_bytes = 0;
+    if (IMPL != IMPL_GLOBAL) {
+        args.cap_bytes = (IMPL == IMPL_COOP ? 48u : 36u) * 1024u * (REAL ? 1u : 2u);
+        smem = args.cap_bytes + (IMPL == IMPL_COOP ? (uint32_t)SPF_COOP_WTS_BYTES : 0u);
+        SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
     const int64_t blocks = args.n_patches * args.M;
     if (blocks > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: M * patches exceeds 2^31-1 blocks; split M");
     int rc = spf_record_event(ctx, 0, st);
     if (rc) return rc;
-    kern<<<(unsigned)blocks, SPF_PATCH, STAGED ? smem : 0, st>>>(args);
+    kern<<<(unsigned)blocks, SPF_PATCH, smem, st>>>(args);
     SPF_LAUNCH_CHECK(ctx);
     if ((rc = spf_record_event(ctx, 1, st))) return rc;
     ctx->ev_valid[0] = ctx->opt_record_events != 0;
     return SPF_OK;
 }
 
-template <int W, bool REAL, int OUTK>
-int launch_slice_impl(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, bool staged, cudaStream_t st) {
-    return staged ? launch_slice<W, REAL, OUTK, true>(ctx, args, smem, st) : launch_slice<W, REAL, OUTK, false>(ctx, args, smem, st);
-}
-
 template <bool REAL, int OUTK>
-int launch_slice_w(spf_ctx *ctx, const SliceArgs &args, uint32_t smem, bool staged, cudaStream_t st) {
+int launch_slice_w(spf_ctx *ctx, SliceArgs &args, int impl, cudaStream_t st) {
     switch (ctx->w) {
-        case 7: return launch_slice_impl<7, REAL, OUTK>(ctx, args, smem, staged, st);
-        case 10: return launch_slice_impl<10, REAL, OUTK>(ctx, args, smem, staged, st);
-        default: return launch_slice<0, REAL, OUTK, false>(ctx, args, smem, st);  // any other width: runtime-w global gather
+        case 7:
+            if (impl == IMPL_COOP) return launch_slice<7, REAL, OUTK, IMPL_COOP>(ctx, args, st);
+            if (impl == IMPL_STAGED) return launch_slice<7, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
+            return launch_slice<7, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
+        case 10:   // 10 x 10 window: the cooperative form (8 x 8) does not apply
+            if (impl != IMPL_GLOBAL) return launch_slice<10, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
+            return launch_slice<10, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
+        default: return launch_slice<0, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);  // any other width: runtime-w global gather
     }
 }
 
@@ -235,14 +296,12 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.beta = (float)ctx->beta;
     args.deg = spfm::fit_kernel_polys(ctx->w, ctx->beta, args.coef);
     args.maps = real ? ctx->maps_r : ctx->maps_c;
-    const uint32_t smem = real ? 36u * 1024u : 72u * 1024u;
-    args.cap_bytes = smem;
     args.fault = ctx->d_fault;
-    const bool staged = (ctx->opt_slice_impl == 0);
+    const int impl = ctx->opt_slice_impl;
     if (real) {
-        return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<true, SPF_OUT_COMPLEX>(ctx, args, smem, staged, st)
-                                           : launch_slice_w<true, SPF_OUT_INTENSITY>(ctx, args, smem, staged, st);
+        return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<true, SPF_OUT_COMPLEX>(ctx, args, impl, st)
+                                           : launch_slice_w<true, SPF_OUT_INTENSITY>(ctx, args, impl, st);
     }
-    return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<false, SPF_OUT_COMPLEX>(ctx, args, smem, staged, st)
-                                       : launch_slice_w<false, SPF_OUT_INTENSITY>(ctx, args, smem, staged, st);
+    return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<false, SPF_OUT_COMPLEX>(ctx, args, impl, st)
+                                       : launch_slice_w<false, SPF_OUT_INTENSITY>(ctx, args, impl, st);
 }

@@ -27,6 +27,13 @@
 #endif
 #define SPF_MAX_DEG 12
 
+// Menu of TMA box sizes of the staged slicing kernels: {SPF_BOX_MIN, +SPF_BOX_STEP, ..., SPF_BOX_MAX}
+// cells along z and along y, one x-plane deep; one tensor map per (by, bz) pair.
+#define SPF_BOX_MIN 8
+#define SPF_BOX_MAX 40
+#define SPF_BOX_STEP 4
+#define SPF_BOX_N ((SPF_BOX_MAX - SPF_BOX_MIN) / SPF_BOX_STEP + 1)  // 9
+
 namespace spfm {
 
 struct alignas(8) c2 { float x, y; };
@@ -120,6 +127,88 @@ SPF_HD c2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMA
         if (!REAL) acci = fmaf(wx[t1], pi, acci);
     }
     c2 r; r.x = accr; r.y = acci;
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------
+// shared-memory tile of the staged kernels (k_slice, slice_impl 0 and 2) and the cooperative gather
+// ------------------------------------------------------------------------------------------
+// A block's points touch the box [lo, hi + w) of padded cells; L = hi - lo + w per axis.  The box is
+// staged one x-plane per TMA copy with a (by x bz)-cell box taken from a fixed menu (one tensor map
+// per size), rows written densely (row pitch = bz cells), planes S1 cells apart (128-byte aligned).
+//   per-lane gather (coop = false): by, bz = L rounded up to the menu step.
+//   cooperative gather (coop = true, w <= 8): a warp's lanes read rows t2 = h, h + 4 (h = lane >> 3)
+//     and cells t3 = lane & 7 of every x-plane, i.e. an 8 x 8 window per point, so the box needs
+//     8 - w spare rows and cells; bz is 8, 24 or 40 (bz = 8 mod 16), which puts the four rows a warp
+//     reads at once (offsets 0, bz, 2 bz, 3 bz) into four disjoint groups of 8 banks: no conflicts.
+struct TileGeom { int by, bz, S1; bool ok; };
+SPF_HD TileGeom tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, uint32_t cap_bytes, bool coop) {
+    TileGeom g;
+    const int ey = coop ? Ly + 8 - w : Ly, ez = coop ? Lz + 8 - w : Lz;
+    g.by = (ey + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP;
+    if (g.by < SPF_BOX_MIN) g.by = SPF_BOX_MIN;
+    if (coop) g.bz = ez <= 8 ? 8 : (ez <= 24 ? 24 : 40);
+    else {
+        g.bz = (ez + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP;
+        if (g.bz < SPF_BOX_MIN) g.bz = SPF_BOX_MIN;
+    }
+    const int per128 = 128 / cell_bytes;
+    g.S1 = (g.by * g.bz + per128 - 1) / per128 * per128;
+    g.ok = Lx > 0 && g.by <= SPF_BOX_MAX && g.bz <= SPF_BOX_MAX && ez <= SPF_BOX_MAX &&
+           (uint64_t)Lx * (uint64_t)g.S1 * (uint64_t)cell_bytes <= (uint64_t)cap_bytes;
+    return g;
+}
+SPF_HD int tile_map_index(int by, int bz) { return ((by - SPF_BOX_MIN) / SPF_BOX_STEP) * SPF_BOX_N + (bz - SPF_BOX_MIN) / SPF_BOX_STEP; }
+
+// One point's 3 w weights as the cooperative gather reads them (SPF_COOP_STRIDE floats per point; the
+// stride of 28 keeps the owners' 16-byte stores and the warp's loads free of bank conflicts):
+//   [0,8)   wz[0..7]                       (0 beyond w)
+//   [8,16)  wy[0],wy[4],wy[1],wy[5],wy[2],wy[6],wy[3],wy[7]   (pairs read as one 8-byte load)
+//   [16,24) wx[0..7]
+#define SPF_COOP_STRIDE 28
+template <int WMAX>
+SPF_HD void coop_pack_weights(float (&out)[24], int w, const float (&wx)[WMAX], const float (&wy)[WMAX], const float (&wz)[WMAX]) {
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {
+        float vx = 0.0f, vy = 0.0f, vz = 0.0f;
+        if (t < WMAX) {
+            if (t < w) { vx = wx[t < WMAX ? t : 0]; vy = wy[t < WMAX ? t : 0]; vz = wz[t < WMAX ? t : 0]; }
+        }
+        out[t] = vz;
+        out[8 + 2 * (t & 3) + (t >> 2)] = vy;
+        out[16 + t] = vx;
+    }
+}
+
+// Partial sum of lane (h, k) for one point: tile = staged box, cell = the point's first cell inside the
+// box (x-plane pitch S1, row pitch bz), wts = the point's weights as stored above.
+//   sum_t1 wx[t1] (wy[h] wz[k] b[t1][h][k] + wy[h+4] wz[k] b[t1][h+4][k])
+// BZ > 0 fixes the row pitch at compile time (the row offsets become immediates); BZ = 0 uses bz.
+template <bool REAL, int BZ>
+SPF_HD c2 gather_coop_lane(const float *tile, int cell, int S1, int bz, int w, const float *wts, int h, int k) {
+    constexpr int E = REAL ? 1 : 2;
+    const int rp = BZ ? BZ : bz;
+    const float wzk = wts[k];
+    const float cA = wts[8 + 2 * h] * wzk, cB = wts[9 + 2 * h] * wzk;
+    const float *p0 = tile + (size_t)(cell + h * rp + k) * E;
+    const size_t row4 = (size_t)(4 * rp) * E, plane = (size_t)S1 * E;
+    float ar = 0.0f, ai = 0.0f, br = 0.0f, bi = 0.0f;
+#pragma unroll 8
+    for (int t1 = 0; t1 < w; ++t1) {
+        const float wxt = wts[16 + t1];
+        if (REAL) {
+            ar = fmaf(wxt, p0[0], ar);
+            br = fmaf(wxt, p0[row4], br);
+        } else {
+            const c2 v0 = *reinterpret_cast<const c2 *>(p0), v1 = *reinterpret_cast<const c2 *>(p0 + row4);
+            ar = fmaf(wxt, v0.x, ar); ai = fmaf(wxt, v0.y, ai);
+            br = fmaf(wxt, v1.x, br); bi = fmaf(wxt, v1.y, bi);
+        }
+        p0 += plane;
+    }
+    c2 r;
+    r.x = fmaf(cA, ar, cB * br);
+    r.y = REAL ? 0.0f : fmaf(cA, ai, cB * bi);
     return r;
 }
 

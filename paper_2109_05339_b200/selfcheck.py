@@ -1,9 +1,10 @@
 """Device self-check of libspf's kernel variants.
 
-libspf has two implementations of each hot kernel: one with the least machinery (plain global
-gather; single-CTA tcgen05 GEMM) and a faster one (TMA-staged shared-memory gather; cta_group::2
-GEMM on CTA pairs).  The library starts on the first; `SpfContext.spf_autotune()` switches on the
-second where this self-check passes on the device at hand.
+libspf has several implementations of each hot kernel: one with the least machinery (plain global
+gather; single-CTA tcgen05 GEMM) and faster ones (TMA-staged shared-memory gather, one thread or one
+warp per point; cta_group::2 GEMM on CTA pairs).  The library starts on the first;
+`SpfContext.spf_autotune()` switches on the faster ones that pass this self-check on the device at
+hand, and among the slicing variants that pass, the one the check timed fastest.
 
 A check runs in a CHILD process (`python -m paper_2109_05339_b200.selfcheck <variant>`): a kernel
 that faults poisons its CUDA context, and the caller's must survive that.  The child compares the
@@ -22,12 +23,13 @@ import subprocess
 import sys
 import time
 
-VARIANTS = ("match_cg1", "slice_staged", "match_cg2")
+VARIANTS = ("match_cg1", "slice_staged", "slice_coop", "match_cg2")
+SLICE_IMPL = {"slice_staged": 0, "slice_coop": 2}
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
 
 
-def _check_slice_staged(device: int) -> str:
+def _check_slice_staged(device: int, impl: int):
     import torch
     from .binding import SpfContext, SPF_OUT_COMPLEX
     dev = torch.device("cuda", device)
@@ -55,8 +57,8 @@ def _check_slice_staged(device: int) -> str:
         ctx.spf_prepare_model(A.to(dev))
         assert bool(ctx.info.grid_is_real) == even
         outs = []
-        for impl in (1, 0):
-            ctx.spf_set_option("slice_impl", impl)
+        for which in (1, impl):
+            ctx.spf_set_option("slice_impl", which)
             outs.append(ctx.spf_slice(quats.to(dev), pix.to(dev), SPF_OUT_COMPLEX))
             ctx.spf_check_fault()
         err = float((outs[1] - outs[0]).abs().pow(2).sum().sqrt() / outs[0].abs().pow(2).sum().sqrt())
@@ -65,7 +67,52 @@ def _check_slice_staged(device: int) -> str:
         if not err <= 3e-6:
             raise AssertionError("staged vs global gather: relative L2 %.3e (n=%d eps=%g)" % (err, n, eps))
         ctx.close()
-    return "staged == global gather to %.1e" % worst
+    return "slice_impl %d == global gather to %.1e" % (impl, worst), _time_slice(device, impl)
+
+
+def _time_slice(device: int, impl: int) -> dict:
+    """Milliseconds of spf_slice for 256 orientations x 16,384 pixels of a 64^3 even model (real grid, w = 7),
+    global gather and variant `impl`, best of 3 (CUDA events on the current stream)."""
+    import torch
+    from .binding import SpfContext, SPF_OUT_INTENSITY
+    dev = torch.device("cuda", device)
+    g = torch.Generator(device="cpu"); g.manual_seed(3)
+    n = 64
+    A = torch.randn((n, n, n), generator=g, dtype=torch.float32)
+    idx = (2 * (n // 2) - torch.arange(n)) % n
+    A = 0.5 * (A + A[idx][:, idx][:, :, idx])
+    A[0] = 0; A[:, 0] = 0; A[:, :, 0] = 0
+    edge = 64
+    t = (torch.arange(edge, dtype=torch.float64) - (edge - 1) / 2) / (2 * edge)
+    pix = []
+    for cy in (-0.26, 0.26):
+        for cx in (-0.26, 0.26):
+            vv, uu = torch.meshgrid(t + cy, t + cx, indexing="ij")
+            k = torch.stack([uu, vv, torch.ones_like(uu)], -1)
+            pix.append((k / k.norm(dim=-1, keepdim=True) - torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64)).reshape(-1, 3))
+    pix = torch.cat(pix)
+    pix = (pix * (0.9 * torch.pi / pix.norm(dim=-1).max())).to(torch.float32).to(dev)
+    quats = torch.randn((256, 4), generator=g, dtype=torch.float32).to(dev)
+    ctx = SpfContext(n, eps=1e-6, device=device)
+    ctx.spf_set_detector_layout(4, edge, edge)
+    ctx.spf_prepare_model(A.to(dev))
+    out = torch.empty((256, pix.shape[0]), dtype=torch.float32, device=dev)
+    ms = {}
+    for which in (1, impl):
+        ctx.spf_set_option("slice_impl", which)
+        best = float("inf")
+        for rep in range(4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.spf_slice(quats, pix, SPF_OUT_INTENSITY, out=out)
+            e1.record()
+            e1.synchronize()
+            if rep:
+                best = min(best, e0.elapsed_time(e1))
+        ctx.spf_check_fault()
+        ms["global" if which == 1 else "variant"] = best
+    ctx.close()
+    return {"slice_ms_global": ms["global"], "slice_ms": ms["variant"], "points": 256 * int(pix.shape[0])}
 
 
 def _check_match(device: int, cta_group: int) -> str:
@@ -101,13 +148,14 @@ def _check_match(device: int, cta_group: int) -> str:
     return "cta_group::%d == CUDA-core matcher, distances to %.1e" % (cta_group, worst)
 
 
-def run_variant(variant: str, device: int = 0) -> str:
-    if variant == "slice_staged":
-        return _check_slice_staged(device)
+def run_variant(variant: str, device: int = 0):
+    """Returns (one-line description, metrics dict)."""
+    if variant in SLICE_IMPL:
+        return _check_slice_staged(device, SLICE_IMPL[variant])
     if variant == "match_cg1":
-        return _check_match(device, 1)
+        return _check_match(device, 1), {}
     if variant == "match_cg2":
-        return _check_match(device, 2)
+        return _check_match(device, 2), {}
     raise ValueError("unknown variant %r (one of %s)" % (variant, ", ".join(VARIANTS)))
 
 
@@ -121,8 +169,31 @@ def check_in_child(variant: str, device: int = 0, timeout_s: float = 240.0) -> d
     except subprocess.TimeoutExpired as e:
         status, out = -999, (e.stdout or "") if isinstance(e.stdout, str) else ""
         out += "\n[selfcheck] timed out after %.0f s" % timeout_s
-    tail = [ln for ln in out.strip().splitlines() if ln.strip()][-3:]
-    return {"ok": status == 0, "status": status, "detail": " | ".join(tail)[-400:], "seconds": round(time.time() - t0, 1)}
+    lines = [ln for ln in out.strip().splitlines() if ln.strip()]
+    metrics = {}
+    for ln in lines:
+        if ln.startswith("[selfcheck-json] "):
+            try:
+                metrics = json.loads(ln[len("[selfcheck-json] "):])
+            except ValueError:
+                pass
+    tail = [ln for ln in lines if not ln.startswith("[selfcheck-json] ")][-3:]
+    return {"ok": status == 0, "status": status, "detail": " | ".join(tail)[-400:], "seconds": round(time.time() - t0, 1),
+            "metrics": metrics}
+
+
+def fastest_slice_impl(report: dict) -> int:
+    """slice_impl to use given a verified_variants report: the verified variant with the lowest timed
+    spf_slice, provided it beat the global gather in its own child's timing; else 1 (global gather)."""
+    best, best_ms = 1, None
+    for v, impl in SLICE_IMPL.items():
+        r = report.get(v) or {}
+        m = r.get("metrics") or {}
+        if not r.get("ok") or "slice_ms" not in m:
+            continue
+        if m["slice_ms"] < m.get("slice_ms_global", float("inf")) and (best_ms is None or m["slice_ms"] < best_ms):
+            best, best_ms = impl, m["slice_ms"]
+    return best
 
 
 def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = None) -> dict:
@@ -153,7 +224,9 @@ if __name__ == "__main__":
         print(json.dumps(rep))
         sys.exit(0 if all(r["ok"] for r in rep.values()) else 1)
     try:
-        print("[selfcheck] %s: %s" % (a.variant, run_variant(a.variant, a.device)))
+        text, metrics = run_variant(a.variant, a.device)
+        print("[selfcheck-json] " + json.dumps(metrics))
+        print("[selfcheck] %s: %s" % (a.variant, text))
     except Exception as e:   # disagreement, SPF_EFAULT from the watchdog, CUDA error
         print("[selfcheck] %s FAILED: %s: %s" % (a.variant, type(e).__name__, e))
         sys.exit(1)

@@ -5,6 +5,11 @@
 // k_slice (spf_slice.cu): rotate in fp64 -> cell + fraction -> 3 w weights -> gather.
 //
 // Build: g++ -O2 -fopenmp -fPIC -shared -std=c++17 -ffp-contract=off spf_hostsim.cpp -o libspf_hostsim.so
+#include <limits.h>
+
+#include <algorithm>
+#include <cmath>
+
 #include "../../paper_2109_05339_b200/csrc/spf_slice_math.cuh"
 
 extern "C" {
@@ -55,6 +60,119 @@ void hostsim_slice(const float *grid, int is_real, int np, int sz, int nf, int h
             out[2 * (m * P + j) + 1] = c.y;
         }
     }
+}
+
+// Replay of one k_slice<STAGED | COOP> launch on the CPU, block by block (spf_slice.cu): patch table ->
+// per-point cell + fraction -> block bounding box -> tile_geom -> the tile image TMA would write (one
+// (by x bz) box per x-plane at pitch S1, zeros outside the padded grid) -> gather from the tile, either
+// one thread per point (coop = 0) or lane by lane as a warp does it (coop = 1: weights parked in the
+// 28-float layout, 32 partial sums added in the shuffle tree's order).  Everything the tile image
+// does NOT receive from a copy is NaN, so a read outside the staged box poisons the result even
+// where its weight is zero.  stats: [0] blocks staged, [1] blocks not staged (global gather),
+// [2] largest tile in bytes.
+void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf, int halo, int w, const float *quats, long M,
+                          const float *pix, long P, const int *patch, long n_patches, int coop, unsigned cap_bytes,
+                          float *out, long *stats) {
+    static float coef[SPF_MAX_W][SPF_MAX_DEG + 1];
+    const double beta = 2.30 * w;
+    const int deg = spfm::fit_kernel_polys(w, beta, coef);
+    const double kPi = 3.14159265358979323846;
+    const double xi_scale = (double)nf / (2.0 * kPi), inv_nf = 1.0 / (double)nf;
+    const int off = nf / 2 + halo;
+    const int E = is_real ? 1 : 2, CELL = 4 * E;
+    const int PATCH = 128;
+    long n_staged = 0, n_global = 0, max_tile = 0;
+#pragma omp parallel for schedule(dynamic) reduction(+ : n_staged, n_global) reduction(max : max_tile)
+    for (long blk = 0; blk < M * n_patches; ++blk) {
+        const long m = blk / n_patches, pt = blk % n_patches;
+        double R[9];
+        spfm::quat_to_R(quats + 4 * m, R);
+        int px[PATCH], py[PATCH], pz[PATCH];
+        long jj[PATCH];
+        float wx[PATCH][SPF_MAX_W], wy[PATCH][SPF_MAX_W], wz[PATCH][SPF_MAX_W];
+        int lo[3] = {INT_MAX, INT_MAX, INT_MAX}, hi[3] = {INT_MIN, INT_MIN, INT_MIN};
+        for (int t = 0; t < PATCH; ++t) {
+            const long j = patch[pt * PATCH + t];
+            jj[t] = j;
+            if (j < 0) continue;
+            const double q0 = pix[3 * j], q1 = pix[3 * j + 1], q2 = pix[3 * j + 2];
+            float fx, fy, fz;
+            spfm::cell_and_fraction(R[0] * q0 + R[1] * q1 + R[2] * q2, xi_scale, inv_nf, nf, off, np, w, px[t], fx);
+            spfm::cell_and_fraction(R[3] * q0 + R[4] * q1 + R[5] * q2, xi_scale, inv_nf, nf, off, np, w, py[t], fy);
+            spfm::cell_and_fraction(R[6] * q0 + R[7] * q1 + R[8] * q2, xi_scale, inv_nf, nf, off, np, w, pz[t], fz);
+            spfm::weights_poly<SPF_MAX_W>(fx, w, coef, deg, wx[t]); spfm::weights_poly<SPF_MAX_W>(fy, w, coef, deg, wy[t]);
+            spfm::weights_poly<SPF_MAX_W>(fz, w, coef, deg, wz[t]);
+            lo[0] = std::min(lo[0], px[t]); hi[0] = std::max(hi[0], px[t]);
+            lo[1] = std::min(lo[1], py[t]); hi[1] = std::max(hi[1], py[t]);
+            lo[2] = std::min(lo[2], pz[t]); hi[2] = std::max(hi[2], pz[t]);
+        }
+        const bool any = hi[0] >= lo[0];
+        const int Lx = any ? hi[0] - lo[0] + w : 0, Ly = any ? hi[1] - lo[1] + w : 0, Lz = any ? hi[2] - lo[2] + w : 0;
+        const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, cap_bytes, coop != 0);
+        std::vector<float> tile;
+        if (g.ok) {
+            n_staged++;
+            max_tile = std::max(max_tile, (long)Lx * g.S1 * CELL);
+            tile.assign((size_t)(cap_bytes / 4) + 8192, std::nanf(""));   // slack: a stray read must find NaN, not crash
+            for (int x = 0; x < Lx; ++x)          // one TMA copy per x-plane: box (bz*E floats, by rows, 1 plane)
+                for (int y = 0; y < g.by; ++y)
+                    for (int z = 0; z < g.bz * E; ++z) {
+                        const long gx = lo[0] + x, gy = lo[1] + y, gz = (long)lo[2] * E + z;
+                        const bool in = gx < np && gy < np && gz < (long)sz * E;   // TMA fills out-of-range elements with zeros
+                        tile[(size_t)x * g.S1 * E + (size_t)y * g.bz * E + z] = in ? grid[((size_t)gx * np + gy) * sz * E + gz] : 0.0f;
+                    }
+        } else {
+            n_global++;
+        }
+        spfm::c2 res[PATCH];
+        if (g.ok && coop) {
+            std::vector<float> wts((size_t)PATCH * SPF_COOP_STRIDE, std::nanf(""));
+            for (int t = 0; t < PATCH; ++t) {
+                float pk[24];
+                spfm::coop_pack_weights<SPF_MAX_W>(pk, w, wx[t], wy[t], wz[t]);
+                for (int v = 0; v < 24; ++v) wts[(size_t)t * SPF_COOP_STRIDE + v] = jj[t] >= 0 ? pk[v] : std::nanf("");
+            }
+            for (int t = 0; t < PATCH; ++t) {
+                if (jj[t] < 0) continue;
+                const int cell = (px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2]);
+                float pr[32], pi[32];
+                for (int lane = 0; lane < 32; ++lane) {
+                    const spfm::c2 c = is_real ? spfm::gather_coop_lane<true, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7)
+                                               : spfm::gather_coop_lane<false, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7);
+                    pr[lane] = c.x; pi[lane] = c.y;
+                }
+                for (int o = 16; o > 0; o >>= 1)      // xor butterfly: every lane ends with the same sum
+                    for (int lane = 0; lane < 32; ++lane)
+                        if (!(lane & o)) {
+                            const float a = pr[lane] + pr[lane ^ o], b = pi[lane] + pi[lane ^ o];
+                            pr[lane] = pr[lane ^ o] = a; pi[lane] = pi[lane ^ o] = b;
+                        }
+                res[t].x = pr[t & 31]; res[t].y = pi[t & 31];
+            }
+        } else {
+            for (int t = 0; t < PATCH; ++t) {
+                if (jj[t] < 0) continue;
+                if (g.ok) {
+                    const float *base = tile.data() + (size_t)((px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2])) * E;
+                    res[t] = is_real ? spfm::gather<SPF_MAX_W, true>(base, g.S1, g.bz, w, wx[t], wy[t], wz[t])
+                                     : spfm::gather<SPF_MAX_W, false>(base, g.S1, g.bz, w, wx[t], wy[t], wz[t]);
+                } else {
+                    const float *base = grid + ((size_t)((size_t)px[t] * np + py[t]) * sz + pz[t]) * E;
+                    res[t] = is_real ? spfm::gather<SPF_MAX_W, true>(base, np * sz, sz, w, wx[t], wy[t], wz[t])
+                                     : spfm::gather<SPF_MAX_W, false>(base, np * sz, sz, w, wx[t], wy[t], wz[t]);
+                }
+            }
+        }
+        for (int t = 0; t < PATCH; ++t)
+            if (jj[t] >= 0) { out[2 * (m * P + jj[t])] = res[t].x; out[2 * (m * P + jj[t]) + 1] = res[t].y; }
+    }
+    stats[0] = n_staged; stats[1] = n_global; stats[2] = max_tile;
+}
+
+// tile geometry alone, for the menu / capacity tests
+void hostsim_tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, unsigned cap, int coop, int *out4) {
+    const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, cell_bytes, cap, coop != 0);
+    out4[0] = g.by; out4[1] = g.bz; out4[2] = g.S1; out4[3] = g.ok ? 1 : 0;
 }
 
 // cell index and fraction of one coordinate, for the index-range tests

@@ -1,7 +1,7 @@
 """GPU parity of the faster kernel variants (-m gpu; collected after tests/test_gpu_parity.py).
 
-`slice_impl = 0` (TMA-staged shared-memory gather) and `match_cta_group = 2` (tcgen05 on CTA pairs)
-are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
+`slice_impl = 0` / `2` (TMA-staged shared-memory gather, one thread / one warp per point) and
+`match_cta_group = 2` (tcgen05 on CTA pairs) are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
 distances <= 1e-4, argmin exact outside near-ties.  Before a variant is launched in this process its
 device self-check (paper_2109_05339_b200/selfcheck.py) must have passed in a child process; if it did
 not, the test fails there, with the child's report, without launching the variant here.
@@ -33,21 +33,26 @@ def _require(verified, variant):
         pytest.fail("device self-check of %s did not pass (status %s): %s" % (variant, r["status"], r["detail"]))
 
 
-@pytest.mark.parametrize("variant", ["match_cg1", "slice_staged", "match_cg2"])
+@pytest.mark.parametrize("variant", ["match_cg1", "slice_staged", "slice_coop", "match_cg2"])
 def test_variant_selfcheck(verified, variant):
     _require(verified, variant)
 
 
 # --------------------------------------------------------------------------------- staged slicing
 
+STAGED = [("slice_staged", 0), ("slice_coop", 2)]
+
+
+@pytest.mark.parametrize("variant,impl", STAGED)
 @pytest.mark.parametrize("force_complex,layout", [(0, True), (1, True), (0, False), (1, False)])
-def test_staged_slice_tiny_full(spf, tiny, verified, force_complex, layout):
-    _require(verified, "slice_staged")
-    base.slice_tiny_full(spf, tiny, 0, force_complex, layout)
+def test_staged_slice_tiny_full(spf, tiny, verified, force_complex, layout, variant, impl):
+    _require(verified, variant)
+    base.slice_tiny_full(spf, tiny, impl, force_complex, layout)
 
 
 def test_staged_slice_equals_the_layout_free_result(spf, tiny, verified):
-    """Patch shape only changes which tile is staged, never the value: bit-identical outputs."""
+    """Patch shape only changes which tile is staged, never the value: bit-identical outputs (one thread per
+    point; the warp-per-point form adds its partial sums in a fixed lane order, so it is layout-free too)."""
     _require(verified, "slice_staged")
     cfg, model, pix, refs, _ = tiny
     outs = []
@@ -61,17 +66,18 @@ def test_staged_slice_equals_the_layout_free_result(spf, tiny, verified):
     assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
 
 
+@pytest.mark.parametrize("variant,impl", STAGED)
 @pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9)])
-def test_staged_slice_general_model(spf, verified, N, eps):
-    """Non-even model (complex fine grid), even and odd N, w = 7 and w = 10."""
-    _require(verified, "slice_staged")
+def test_staged_slice_general_model(spf, verified, N, eps, variant, impl):
+    """Non-even model (complex fine grid), even and odd N, w = 7 and w = 10 (w = 10 runs one thread per point)."""
+    _require(verified, variant)
     rng = np.random.default_rng(4)
     A = rng.standard_normal((N, N, N)).astype(np.float32)
     pix = make_detector(1, 16)
     refs = random_quaternions(9, seed=31)
     c_ref = orc.slice_points(A, refs, pix)
     ctx = spf.SpfContext(N, eps=eps)
-    ctx.spf_set_option("slice_impl", 0)
+    ctx.spf_set_option("slice_impl", impl)
     ctx.spf_set_detector_layout(1, 16, 16)
     ctx.spf_prepare_model(_dev(A))
     c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy()
@@ -79,15 +85,16 @@ def test_staged_slice_general_model(spf, verified, N, eps):
     assert _rel_l2(c, c_ref) <= max(SLICE_TOL, 10 * eps)
 
 
-def test_staged_slice_small_config_sampled(spf, verified):
-    """Small (configs[1]) through the staged kernel, real and complex grid, 4,096 oracle samples."""
-    _require(verified, "slice_staged")
+@pytest.mark.parametrize("variant,impl", STAGED)
+def test_staged_slice_small_config_sampled(spf, verified, variant, impl):
+    """Small (configs[1]) through the staged kernels, real and complex grid, 4,096 oracle samples."""
+    _require(verified, variant)
     cfg = CONFIGS["small"]
     model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
     pix = make_detector(cfg.panels, cfg.panel_edge)
     refs = random_quaternions(cfg.M, seed=2)
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
-    ctx.spf_set_option("slice_impl", 0)
+    ctx.spf_set_option("slice_impl", impl)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
     ctx.spf_prepare_model(_dev(model))
     sm, sj = sample_pairs(cfg.M, cfg.P, 4096)

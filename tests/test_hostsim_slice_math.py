@@ -34,6 +34,9 @@ def sim():
     L.hostsim_slice.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_long,
                                 C.c_void_p, C.c_long, C.c_int, C.c_void_p]
     L.hostsim_cell.argtypes = [C.c_double, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+    L.hostsim_slice_blocks.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_long,
+                                       C.c_void_p, C.c_long, C.c_void_p, C.c_long, C.c_int, C.c_uint, C.c_void_p, C.c_void_p]
+    L.hostsim_tile_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_int, C.c_void_p]
     return L
 
 
@@ -173,3 +176,159 @@ def test_paper_scale_sampled_vs_oracle(sim):
     err = _rel(c[sm, sj].real, ref.real)
     print("paper-scale host-compiled slice arithmetic vs oracle: rel L2 %.3e" % err)
     assert err <= SLICE_TOL
+
+
+# ------------------------------------------------------------------------------------------------
+# staged kernels (slice_impl 0 and 2): block-level replay of the tile staging and of the warp-per-point gather
+# ------------------------------------------------------------------------------------------------
+def _patch_table(panels, rows, cols, P):
+    """build_patches (spf_slice.cu): 8 x 16 lattice tiles per panel under a layout promise, else runs of 128."""
+    tab = []
+    if panels:
+        for p in range(panels):
+            for r0 in range(0, rows, 8):
+                for c0 in range(0, cols, 16):
+                    for t in range(128):
+                        r, c = r0 + t // 16, c0 + t % 16
+                        tab.append((p * rows + r) * cols + c if (r < rows and c < cols) else -1)
+    else:
+        n = (P + 127) // 128
+        tab = [i if i < P else -1 for i in range(n * 128)]
+    return np.asarray(tab, np.int32)
+
+
+def _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, quats, pix, table, coop):
+    grid = np.ascontiguousarray(g.real.astype(np.float32)) if is_real else np.ascontiguousarray(g).view(np.float32)
+    quats, pix = np.ascontiguousarray(quats, np.float32), np.ascontiguousarray(pix, np.float32)
+    out = np.full((quats.shape[0], pix.shape[0]), np.nan + 0j, np.complex64)
+    stats = np.zeros(3, np.int64)
+    cap = (48 if coop else 36) * 1024 * (1 if is_real else 2)        # launch_slice (spf_slice.cu)
+    sim.hostsim_slice_blocks(grid.ctypes.data, int(is_real), npad, sz, nf, halo, w, quats.ctypes.data, quats.shape[0],
+                             pix.ctypes.data, pix.shape[0], table.ctypes.data, len(table) // 128, int(coop), cap,
+                             out.ctypes.data, stats.ctypes.data)
+    return out, stats
+
+
+@pytest.mark.parametrize("coop,is_real,layout", [(1, 1, True), (1, 0, True), (0, 1, True), (1, 1, False), (0, 0, False)])
+def test_staged_block_replay_tiny_full_vs_oracle(sim, coop, is_real, layout):
+    """Tiny through the staged data path: every block's tile image holds NaN wherever no TMA copy writes,
+    so a finite result within tolerance shows every read (zero-weight window padding included) stays
+    inside the staged box, and that the tile indexing and the lane decomposition add up to the w^3 sum."""
+    cfg = CONFIGS["tiny"]
+    A = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(cfg.M, seed=2)
+    w, nf, halo = _plan(cfg.N, cfg.eps)
+    g, npad, sz = _padded_grid(sim, A, w, nf, halo)
+    table = _patch_table(1, 32, 32, cfg.P) if layout else _patch_table(0, 0, 0, cfg.P)
+    c, stats = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, coop)
+    assert np.isfinite(c.view(np.float32)).all()
+    assert stats[0] > 0 and stats[0] + stats[1] == cfg.M * (len(table) // 128)
+    ref = orc.slice_points(A, refs, pix)
+    assert _rel(c.real if is_real else c, ref.real if is_real else ref) <= SLICE_TOL
+    # and it is the same arithmetic as the one-thread-per-point gather from the whole grid, up to summation order
+    direct = _slice(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, 1)
+    assert _rel(c, direct) <= 2e-6
+
+
+def test_staged_block_replay_ragged_patch_and_complex_general_model(sim):
+    """Ragged last patch (P not a multiple of 128) and a non-even model on the complex grid, N even."""
+    rng = np.random.default_rng(4)
+    N = 16
+    A = rng.standard_normal((N, N, N)).astype(np.float32)
+    pix = make_detector(1, 16)[:200]
+    refs = random_quaternions(5, seed=31)
+    w, nf, halo = _plan(N, 1e-6)
+    g, npad, sz = _padded_grid(sim, A, w, nf, halo)
+    table = _patch_table(0, 0, 0, 200)
+    ref = orc.slice_points(A, refs, pix)
+    for coop in (0, 1):
+        c, stats = _slice_blocks(sim, g, 0, npad, sz, nf, halo, w, refs, pix, table, coop)
+        assert np.isfinite(c.view(np.float32)).all() and stats[0] > 0
+        assert _rel(c, ref) <= SLICE_TOL
+
+
+def test_staged_block_replay_paper_scale_sampled(sim):
+    """Paper-scale model and detector (8 x 16 lattice patches of 4 x 128 x 128 pixels), 4 orientations through the
+    warp-per-point path: every block must fit the 48 KB tile (no fallback), 2,048 sampled pairs from the oracle."""
+    cfg = CONFIGS["paper_scale"]
+    A = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(4, seed=2)
+    w, nf, halo = _plan(cfg.N, cfg.eps)
+    g, npad, sz = _padded_grid(sim, A, w, nf, halo)
+    table = _patch_table(cfg.panels, cfg.panel_edge, cfg.panel_edge, cfg.P)
+    c, stats = _slice_blocks(sim, g, 1, npad, sz, nf, halo, w, refs, pix, table, 1)
+    assert stats[1] == 0 and stats[2] <= 48 * 1024, stats
+    assert np.isfinite(c.view(np.float32)).all()
+    sm, sj = sample_pairs(4, cfg.P, 2048)
+    ref = orc.slice_points(A, refs, pix, sm, sj)
+    err = _rel(c[sm, sj].real, ref.real)
+    print("paper-scale warp-per-point replay vs oracle: rel L2 %.3e; largest tile %d bytes" % (err, stats[2]))
+    assert err <= SLICE_TOL
+
+
+def test_tile_geometry_menu_and_bank_rule(sim):
+    """tile_geom: an accepted box is on the tensor-map menu, covers the points' footprint (plus the 8 x 8 window's
+    spare row and cell in the cooperative form), keeps x-planes 128-byte aligned, fits the capacity, and in the
+    cooperative form has a row pitch of 8 mod 16 cells -- the four rows a warp reads at once then fall into four
+    disjoint groups of 8 banks (real grid) or, per half-warp, two disjoint groups of 16 banks (complex grid)."""
+    out = (C.c_int * 4)()
+    for coop in (0, 1):
+        for cell in (4, 8):
+            cap = (48 if coop else 36) * 1024 * (cell // 4)
+            for Lx in (7, 13, 22, 30):
+                for Ly in range(7, 45):
+                    for Lz in range(7, 45):
+                        sim.hostsim_tile_geom(Lx, Ly, Lz, 7, cell, cap, coop, out)
+                        by, bz, S1, ok = out[0], out[1], out[2], out[3]
+                        if not ok:
+                            assert by > 40 or bz > 40 or Lz + coop > 40 or Lx * S1 * cell > cap
+                            continue
+                        assert by in range(8, 41, 4) and bz in range(8, 41, 4)
+                        assert by >= Ly + coop and bz >= Lz + coop and S1 >= by * bz and (S1 * cell) % 128 == 0
+                        assert Lx * S1 * cell <= cap
+                        if coop:
+                            assert bz % 16 == 8
+                            if cell == 4:
+                                banks = sorted((h * bz + k) % 32 for h in range(4) for k in range(8))
+                                assert banks == list(range(32))
+                            else:
+                                for half in (0, 2):
+                                    words = sorted(((h * bz + k) * 2 + e) % 32 for h in (half, half + 1) for k in range(8) for e in (0, 1))
+                                    assert words == list(range(32))
+
+
+def test_bank_conflicts_thread_per_point_vs_warp_per_point():
+    """Why slice_impl 2 exists.  With one thread per point the 32 lanes of a warp read, at
+    every tap, 32 words whose tile addresses follow the rotated pixel lattice -- generic orientations spread them
+    over the 32 banks like random throws, and the load replays max-bank-multiplicity times.  Paper-scale
+    geometry, seeded orientations: the mean replay factor is above 3, i.e. 343 x 3.5 / 32 = 38 shared-memory
+    wavefronts per point, against 14 + 4 for the warp-per-point form whose lanes read 32 consecutive-bank words."""
+    cfg = CONFIGS["paper_scale"]
+    pix = make_detector(cfg.panels, cfg.panel_edge).astype(np.float64)
+    w, nf, halo = _plan(cfg.N, cfg.eps)
+    off = nf // 2 + halo
+    rng = np.random.default_rng(0)
+    degs = []
+    for q in random_quaternions(12, seed=9).astype(np.float64):
+        qw, x, y, z = q / np.linalg.norm(q)
+        R = np.array([[1 - 2 * (y * y + z * z), 2 * (x * y - qw * z), 2 * (x * z + qw * y)],
+                      [2 * (x * y + qw * z), 1 - 2 * (x * x + z * z), 2 * (y * z - qw * x)],
+                      [2 * (x * z - qw * y), 2 * (y * z + qw * x), 1 - 2 * (x * x + y * y)]])
+        i0 = (np.ceil((pix @ R.T) * nf / (2 * np.pi) - w / 2).astype(int) + off).reshape(cfg.panels, cfg.panel_edge, cfg.panel_edge, 3)
+        for _ in range(40):
+            p, r0, c0 = rng.integers(cfg.panels), 8 * rng.integers(cfg.panel_edge // 8), 16 * rng.integers(cfg.panel_edge // 16)
+            t = i0[p, r0:r0 + 8, c0:c0 + 16].reshape(-1, 3)
+            lo = t.min(0)
+            L = t.max(0) - lo + w
+            by, bz = max(8, (L[1] + 3) // 4 * 4), max(8, (L[2] + 3) // 4 * 4)
+            S1 = (by * bz + 31) // 32 * 32
+            addr = (t[:, 0] - lo[0]) * S1 + (t[:, 1] - lo[1]) * bz + (t[:, 2] - lo[2])
+            for wv in range(4):
+                a = addr[32 * wv:32 * wv + 32]
+                degs.append(max(len(set(a[a % 32 == b])) for b in set(a % 32)))
+    mean = float(np.mean(degs))
+    print("thread-per-point staged gather: mean bank-conflict degree %.2f over %d warps" % (mean, len(degs)))
+    assert 3.0 < mean < 4.5
+    assert w ** 3 * mean / 32 > 2 * (2 * w + 4)
