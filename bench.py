@@ -331,9 +331,10 @@ def run_spf(args, cfg):
 def roofline_objects(cfg, info, k_ms, products, peaks, clk):
     """Per-kernel roofline entries from the library's CUDA-event times.
 
-    slice kernel: bound by the fp32 FMA pipes -- w^3 (real grid) or 2 w^3 (complex grid) FMAs per point is
-      the arithmetic the interpolation cannot avoid; peak = SMs x 128 lanes x 2 flop x max SM clock.  The HBM
-      figure (bytes written + the touched part of the grid read once) is reported beside it.
+    slice kernel: bound on chip -- every point needs w^3 grid values brought from shared memory to a lane
+      (128 B/clk/SM) and w^3 (real grid) or 2 w^3 (complex grid) FMAs (128 lanes/clk/SM); the first is the
+      tighter limit by 4x and is the `roofline` entry ("smem"), the FMA-pipe ("alu") and HBM figures (bytes
+      written + the touched part of the grid read once) are reported beside it.
     GEMM: tensor pipe.  achieved = issued MMA flop (all split products); peak = measured sustained bf16 cuBLAS
       throughput (fp16 and bf16 share one rate).  The fp32-equivalent algorithmic rate is reported beside it.
     """
@@ -347,11 +348,19 @@ def roofline_objects(cfg, info, k_ms, products, peaks, clk):
     n_f = int(info.n_fine)
     ball = (4.0 / 3.0) * np.pi * (0.45 * n_f + w) ** 3 * (4 if real else 8)     # touched part of the fine grid, read once
     hbm_bytes = pts * 4.0 + min(ball, n_f ** 3 * (4.0 if real else 8.0))
+    # SM-side memory roofline (north_star's "memory roofline" as SURVEY.md section 8(d) reads it): every point needs
+    # w^3 grid values (4 B real, 8 B complex) delivered from shared memory / L1 to a lane, against 128 B/clk/SM
+    smem_bytes = pts * (w ** 3) * (4.0 if real else 8.0)
+    smem_peak = info.sm_count * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9                # GB/s
+    smem_ach = smem_bytes / t_s / 1e9
     out["slice"] = {"ms": t_s * 1e3, "points_per_s": pts / t_s,
-                    "roofline": {"kernel": "k_slice", "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
-                                 "frac": ach / alu_peak, "traffic": None,
-                                 "peak_source": "148 SM x 128 FMA lanes x 2 x sm_max_mhz (DESIGN.md)",
-                                 "frac_at_observed_clock": (ach / (alu_peak * clk["sm_mhz"] / peaks["sm_max_mhz"])) if clk.get("sm_mhz") else None},
+                    "roofline": {"kernel": "k_slice", "bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "GB/s",
+                                 "frac": smem_ach / smem_peak, "traffic": None,
+                                 "peak_source": "SM-side memory: 148 SM x 128 B/clk x sm_max_mhz; algorithmic bytes = w^3 grid "
+                                                "values per point (DESIGN.md section 6.1); HBM and FMA-pipe figures beside it",
+                                 "frac_at_observed_clock": (smem_ach / (smem_peak * clk["sm_mhz"] / peaks["sm_max_mhz"])) if clk.get("sm_mhz") else None},
+                    "alu": {"achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
+                            "peak_source": "148 SM x 128 FMA lanes x 2 x sm_max_mhz"},
                     "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / t_s / 1e9, "peak_gbs": peaks["hbm_gbs"],
                             "frac": hbm_bytes / t_s / 1e9 / peaks["hbm_gbs"]}}
     t_g = float(np.mean(k_ms["gemm"])) * 1e-3
