@@ -179,7 +179,7 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *   "slice_impl":  [1] = plain global-memory gather, one thread per point;
  *                  0 = tile staged in shared memory by TMA, one thread per point gathers from it;
  *                  2 = the same tile, a warp per point: 32 lanes read an 8 x 8 window per x-plane with no
- *                      bank conflicts and a shuffle tree adds the partial sums (w <= 8; w = 10 runs as 0)
+ *                      bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; w = 10 runs as 0)
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
  *   "match_cta_group": CTAs per tcgen05 MMA: 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
  * The defaults are the variants with the least machinery; the faster ones (slice_impl 0 / 2, match_cta_group 2) are

@@ -168,19 +168,44 @@ __global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slic
         if (COOP) {
             const int lane = tid & 31, h = lane >> 3, k = lane & 7;
             const float *wts_warp = reinterpret_cast<const float *>(s_dyn) + (tid & ~31) * SPF_COOP_STRIDE;
-            // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates
+            // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates.
+            // Points go in groups of 8: eight independent gathers in flight per lane, then ONE multi-value
+            // butterfly (spfm::MR8_*: 4 + 2 + 1 exchanges halve the value count while halving the lane
+            // group, 2 more finish) instead of eight 5-step reductions; lane 4 u ends with point u's sum.
             auto sweep = [&](auto bz_tag) {
                 constexpr int BZ = decltype(bz_tag)::value;
-                for (int p = 0; p < 32; ++p) {
-                    const int cell_p = __shfl_sync(0xffffffffu, cell, p);
-                    if (cell_p < 0) continue;    // warp-uniform: an empty slot of a ragged patch
-                    spfm::c2 part = spfm::gather_coop_lane<REAL, BZ>(tile, cell_p, S1, bz, w, wts_warp + p * SPF_COOP_STRIDE, h, k);
+                for (int g0 = 0; g0 < 32; g0 += spfm::MR8) {
+                    float pr[spfm::MR8], pi[spfm::MR8];
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) {
-                        part.x += __shfl_xor_sync(0xffffffffu, part.x, o);
-                        if (!REAL) part.y += __shfl_xor_sync(0xffffffffu, part.y, o);
+                    for (int u = 0; u < spfm::MR8; ++u) {
+                        const int cell_p = __shfl_sync(0xffffffffu, cell, g0 + u);
+                        spfm::c2 part; part.x = part.y = 0.0f;
+                        if (cell_p >= 0)    // warp-uniform: skips an empty slot of a ragged patch
+                            part = spfm::gather_coop_lane<REAL, BZ>(tile, cell_p, S1, bz, w, wts_warp + (g0 + u) * SPF_COOP_STRIDE, h, k);
+                        pr[u] = part.x; pi[u] = part.y;
                     }
-                    if (lane == p) c = part;
+#pragma unroll
+                    for (int o = 16, n = spfm::MR8 / 2; n >= 1; o >>= 1, n >>= 1) {
+                        const bool upper = (lane & o) != 0;
+#pragma unroll
+                        for (int v = 0; v < n; ++v) {
+                            const float keep_r = upper ? pr[v + n] : pr[v], send_r = upper ? pr[v] : pr[v + n];
+                            pr[v] = keep_r + __shfl_xor_sync(0xffffffffu, send_r, o);
+                            if (!REAL) {
+                                const float keep_i = upper ? pi[v + n] : pi[v], send_i = upper ? pi[v] : pi[v + n];
+                                pi[v] = keep_i + __shfl_xor_sync(0xffffffffu, send_i, o);
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int o = 2; o >= 1; o >>= 1) {
+                        pr[0] += __shfl_xor_sync(0xffffffffu, pr[0], o);
+                        if (!REAL) pi[0] += __shfl_xor_sync(0xffffffffu, pi[0], o);
+                    }
+                    // the lanes g0 .. g0 + 7 own these points; point u's sum sits in lane mr8_result_lane(u)
+                    const float vr = __shfl_sync(0xffffffffu, pr[0], spfm::mr8_result_lane(lane & (spfm::MR8 - 1)));
+                    const float vi = REAL ? 0.0f : __shfl_sync(0xffffffffu, pi[0], spfm::mr8_result_lane(lane & (spfm::MR8 - 1)));
+                    if ((lane & ~(spfm::MR8 - 1)) == g0) { c.x = vr; c.y = vi; }
                 }
             };
             if (bz == 24) sweep(std::integral_constant<int, 24>{});

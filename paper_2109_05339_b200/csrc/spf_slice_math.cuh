@@ -212,6 +212,15 @@ SPF_HD c2 gather_coop_lane(const float *tile, int cell, int S1, int bz, int w, c
     return r;
 }
 
+// Multi-value warp reduction used by the cooperative gather: every lane holds MR8 = 8 partial sums (one
+// per point of a group).  Exchange step with lane offset o = 16, 8, 4 and n = 4, 2, 1 values: a lane whose
+// bit o is set keeps values [n, 2n) and sends [0, n), the others the opposite, and adds what it receives;
+// after the three steps a lane holds ONE value, the partial sum of point u = 4 bit4 + 2 bit3 + bit2 of
+// its lane number over 4 lanes' worth of partials; two plain butterfly steps (o = 2, 1) finish the sum.
+// 9 exchanges for 8 points instead of 40.
+constexpr int MR8 = 8;
+SPF_HD int mr8_result_lane(int u) { return u << 2; }   // a lane that ends with point u's total (bits 1,0 are free)
+
 // ------------------------------------------------------------------------------------------
 // host side (fp64): kernel, polynomial fit of the weights, deapodisation factors
 // ------------------------------------------------------------------------------------------

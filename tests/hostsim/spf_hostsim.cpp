@@ -66,7 +66,7 @@ void hostsim_slice(const float *grid, int is_real, int np, int sz, int nf, int h
 // per-point cell + fraction -> block bounding box -> tile_geom -> the tile image TMA would write (one
 // (by x bz) box per x-plane at pitch S1, zeros outside the padded grid) -> gather from the tile, either
 // one thread per point (coop = 0) or lane by lane as a warp does it (coop = 1: weights parked in the
-// 28-float layout, 32 partial sums added in the shuffle tree's order).  Everything the tile image
+// 28-float layout, groups of 8 points, partial sums added by the multi-value butterfly).  Everything the tile image
 // does NOT receive from a copy is NaN, so a read outside the staged box poisons the result even
 // where its weight is zero.  stats: [0] blocks staged, [1] blocks not staged (global gather),
 // [2] largest tile in bytes.
@@ -132,23 +132,45 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
                 spfm::coop_pack_weights<SPF_MAX_W>(pk, w, wx[t], wy[t], wz[t]);
                 for (int v = 0; v < 24; ++v) wts[(size_t)t * SPF_COOP_STRIDE + v] = jj[t] >= 0 ? pk[v] : std::nanf("");
             }
-            for (int t = 0; t < PATCH; ++t) {
-                if (jj[t] < 0) continue;
-                const int cell = (px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2]);
-                float pr[32], pi[32];
-                for (int lane = 0; lane < 32; ++lane) {
-                    const spfm::c2 c = is_real ? spfm::gather_coop_lane<true, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7)
-                                               : spfm::gather_coop_lane<false, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7);
-                    pr[lane] = c.x; pi[lane] = c.y;
-                }
-                for (int o = 16; o > 0; o >>= 1)      // xor butterfly: every lane ends with the same sum
-                    for (int lane = 0; lane < 32; ++lane)
-                        if (!(lane & o)) {
-                            const float a = pr[lane] + pr[lane ^ o], b = pi[lane] + pi[lane ^ o];
-                            pr[lane] = pr[lane ^ o] = a; pi[lane] = pi[lane ^ o] = b;
+            // warp by warp, points in groups of MR8, exactly as k_slice<.., IMPL_COOP> walks them
+            for (int wv = 0; wv < PATCH / 32; ++wv)
+                for (int g0 = 0; g0 < 32; g0 += spfm::MR8) {
+                    float pr[32][spfm::MR8], pi[32][spfm::MR8];
+                    for (int u = 0; u < spfm::MR8; ++u) {
+                        const int t = wv * 32 + g0 + u;
+                        for (int lane = 0; lane < 32; ++lane) {
+                            spfm::c2 c; c.x = c.y = 0.0f;
+                            if (jj[t] >= 0) {
+                                const int cell = (px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2]);
+                                c = is_real ? spfm::gather_coop_lane<true, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7)
+                                            : spfm::gather_coop_lane<false, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7);
+                            }
+                            pr[lane][u] = c.x; pi[lane][u] = c.y;
                         }
-                res[t].x = pr[t & 31]; res[t].y = pi[t & 31];
-            }
+                    }
+                    for (int o = 16, n = spfm::MR8 / 2; n >= 1; o >>= 1, n >>= 1) {      // exchange steps: all lanes read, then all write
+                        float nr[32][spfm::MR8], ni[32][spfm::MR8];
+                        for (int lane = 0; lane < 32; ++lane) {
+                            const bool upper = (lane & o) != 0, pupper = ((lane ^ o) & o) != 0;
+                            for (int v = 0; v < n; ++v) {
+                                const float keep_r = upper ? pr[lane][v + n] : pr[lane][v], keep_i = upper ? pi[lane][v + n] : pi[lane][v];
+                                const float recv_r = pupper ? pr[lane ^ o][v] : pr[lane ^ o][v + n], recv_i = pupper ? pi[lane ^ o][v] : pi[lane ^ o][v + n];
+                                nr[lane][v] = keep_r + recv_r; ni[lane][v] = keep_i + recv_i;
+                            }
+                        }
+                        for (int lane = 0; lane < 32; ++lane)
+                            for (int v = 0; v < n; ++v) { pr[lane][v] = nr[lane][v]; pi[lane][v] = ni[lane][v]; }
+                    }
+                    for (int o = 2; o >= 1; o >>= 1) {
+                        float nr[32], ni[32];
+                        for (int lane = 0; lane < 32; ++lane) { nr[lane] = pr[lane][0] + pr[lane ^ o][0]; ni[lane] = pi[lane][0] + pi[lane ^ o][0]; }
+                        for (int lane = 0; lane < 32; ++lane) { pr[lane][0] = nr[lane]; pi[lane][0] = ni[lane]; }
+                    }
+                    for (int u = 0; u < spfm::MR8; ++u) {         // owner lane g0 + u fetches from mr8_result_lane(u)
+                        const int t = wv * 32 + g0 + u;
+                        res[t].x = pr[spfm::mr8_result_lane(u)][0]; res[t].y = pi[spfm::mr8_result_lane(u)][0];
+                    }
+                }
         } else {
             for (int t = 0; t < PATCH; ++t) {
                 if (jj[t] < 0) continue;
