@@ -267,6 +267,8 @@ int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
         args.cap_bytes = (IMPL == IMPL_COOP ? 48u : 36u) * 1024u * (REAL ? 1u : 2u);
         smem = args.cap_bytes + (IMPL == IMPL_COOP ? (uint32_t)SPF_COOP_WTS_BYTES : 0u);
         SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        // three (real grid) or two (complex grid) blocks per SM only fit with the largest shared-memory carve-out
+        SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     }
     const int64_t blocks = args.n_patches * args.M;
     if (blocks > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_slice: M * patches exceeds 2^31-1 blocks; split M");
