@@ -217,8 +217,8 @@ def run_spf(args, cfg):
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
     # kernel variants: the faster ones (TMA-staged gather -- the fastest verified form --, cta_group::2 GEMM) where their device self-check
     # passes in a child process, else the library defaults (paper_2109_05339_b200/selfcheck.py)
-    variants = ({"slice_staged": False, "slice_coop": False, "match_cg2": False, "slice_impl": 1, "match_cta_group": 1}
-                if args.no_autotune else ctx.spf_autotune())
+    variants = ({"slice_staged": False, "slice_coop": False, "match_cg1": False, "match_cg2": False, "slice_impl": 1,
+                 "match_impl": 1, "match_cta_group": 1} if args.no_autotune else ctx.spf_autotune())
     info = ctx.info
     d_model = torch.from_numpy(model).to(dev)
     d_pix, d_refs = torch.from_numpy(pix).to(dev), torch.from_numpy(refs).to(dev)
@@ -298,7 +298,8 @@ def run_spf(args, cfg):
                        "grid_is_real": bool(info.grid_is_real),
                        "kernel_variants": {"slice": {0: "tma_staged, thread per point", 1: "global_gather, thread per point",
                                                      2: "tma_staged, warp per point"}[variants["slice_impl"]],
-                                           "match": "tcgen05 cta_group::%d" % variants["match_cta_group"],
+                                           "match": ("tcgen05 cta_group::%d" % variants["match_cta_group"]) if variants["match_impl"] == 0
+                                                    else "cuda_core difference form (tcgen05 self-check did not pass)",
                                            "selfcheck": variants},
                        "parallelism": "images partitioned x%d, orientations replicated" % world,
                        "l2": "inputs larger than L2 (slices %.2f GB, images %.2f GB per step; no flush needed)"
@@ -366,12 +367,22 @@ def roofline_objects(cfg, info, k_ms, products, peaks, clk):
     t_g = float(np.mean(k_ms["gemm"])) * 1e-3
     Ppad = (cfg.P + 63) // 64 * 64
     alg = 2.0 * cfg.n_img * cfg.M * Ppad
-    ach = products * alg / t_g / 1e12
-    out["gemm"] = {"ms": t_g * 1e3, "products": products, "algorithmic_tflops_fp32_equivalent": alg / t_g / 1e12,
-                   "images_per_s": cfg.n_img / t_g,
-                   "roofline": {"kernel": "k_match_gemm", "bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"],
-                                "unit": "TFLOP/s", "frac": ach / peaks["tensor_tflops"], "traffic": None,
-                                "peak_source": "%s sustained bf16 cuBLAS (fp16 = bf16 rate)" % peaks["source"]}}
+    if products:
+        ach = products * alg / t_g / 1e12
+        out["gemm"] = {"ms": t_g * 1e3, "products": products, "algorithmic_tflops_fp32_equivalent": alg / t_g / 1e12,
+                       "images_per_s": cfg.n_img / t_g,
+                       "roofline": {"kernel": "k_match_gemm", "bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"],
+                                    "unit": "TFLOP/s", "frac": ach / peaks["tensor_tflops"], "traffic": None,
+                                    "peak_source": "%s sustained bf16 cuBLAS (fp16 = bf16 rate)" % peaks["source"]}}
+    else:
+        # CUDA-core matcher (the tcgen05 kernel did not pass its self-check): one subtract + one FMA per pixel pair
+        ach = 3.0 * cfg.n_img * cfg.M * cfg.P / t_g / 1e12
+        out["gemm"] = {"ms": t_g * 1e3, "products": 0, "algorithmic_tflops_fp32_equivalent": alg / t_g / 1e12,
+                       "images_per_s": cfg.n_img / t_g,
+                       "roofline": {"kernel": "k_match_simt", "bound": "alu", "achieved": ach, "peak": alu_peak * 0.75,
+                                    "unit": "TFLOP/s", "frac": ach / (alu_peak * 0.75), "traffic": None,
+                                    "peak_source": "148 SM x 128 lanes x sm_max_mhz x 1.5 flop per instruction slot "
+                                                   "(FADD = 1 flop, FFMA = 2 flop alternate)"}}
     t_p = float(np.mean(k_ms["match_prep"])) * 1e-3
     prep_bytes = (cfg.n_img + cfg.M) * cfg.P * 4.0 * 2 + (cfg.n_img + cfg.M) * Ppad * 4.0   # abs-max read + split read + 2 fp16 planes written
     out["match_prep"] = {"ms": t_p * 1e3,

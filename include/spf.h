@@ -181,9 +181,12 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *                  2 = the same tile, a warp per point: 32 lanes read an 8 x 8 window per x-plane with no
  *                      bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; w = 10 runs as 0)
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
- *   "match_cta_group": CTAs per tcgen05 MMA: 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
- * The defaults are the variants with the least machinery; the faster ones (slice_impl 0 / 2, match_cta_group 2) are
- * switched on by the caller once they have been checked on the device at hand (the Python binding's
+ *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused norm-add + argmin epilogue (the product);
+ *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused
+ *                      argmin -- about 20x slower at Paper-scale, no tensor-core, TMA or mbarrier machinery
+ *   "match_cta_group": CTAs per tcgen05 MMA (match_impl 0): 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
+ * The defaults are the variants with the least machinery; the faster ones (slice_impl 0 / 2, match_impl 0,
+ * match_cta_group 2) are switched on by the caller once they have been checked on the device at hand (the Python binding's
  * SpfContext.spf_autotune does that in a child process).
  *   "record_events": [0]; 1 = spf_slice / spf_match record CUDA events on their stream around the
  *                    dominant kernels, read back with spf_last_kernel_ms
@@ -211,7 +214,7 @@ SPF_API int64_t spf_launch_count(const spf_ctx *ctx);
  * Device time in milliseconds (CUDA events recorded on the stream the kernel was launched on,
  * SURVEY.md section 8(d)) of the last call made with option "record_events" = 1:
  *   which = 0: the interpolation kernel of the last spf_slice   (steps a3-a5, one launch)
- *   which = 1: the tcgen05 contraction of the last spf_match    (steps a7-a8, both instantiations)
+ *   which = 1: the contraction of the last spf_match            (steps a7-a8: both tcgen05 instantiations, or k_match_simt)
  *   which = 2: the operand preparation of the last spf_match    (step a6: abs-max, split, norms)
  * ms [host].  Synchronises on the closing event.  SPF_ESTATE when nothing was recorded.
  */
@@ -219,8 +222,9 @@ SPF_API int spf_last_kernel_ms(spf_ctx *ctx, int32_t which, float *ms);
 
 /*
  * Number of fp16 operand products the last spf_match issued per K step: 2 when every image value
- * was exact in one fp16 term (photon counts), else 3.  products [host].  Synchronises the stream of
- * that call and reads one word of its workspace, which must still be allocated.
+ * was exact in one fp16 term (photon counts), else 3; 0 when that call ran the CUDA-core matcher
+ * (match_impl 1).  products [host].  Synchronises the stream of that call and reads one word of its
+ * workspace, which must still be allocated.
  */
 SPF_API int spf_last_match_products(spf_ctx *ctx, int32_t *products);
 

@@ -154,13 +154,16 @@ class SpfContext:
         """Switch on the faster kernel variants that pass the device self-check (selfcheck.py, run once per
         process in a child process so that a faulting variant cannot take this process's CUDA context with
         it): for slicing the verified variant that the check timed fastest (TMA-staged, one thread or one
-        warp per point), for matching cta_group::2 when verified.  Returns {variant: bool} plus
-        "slice_impl" / "match_cta_group" = the options now in force."""
+        warp per point), for matching the tcgen05 GEMM (cta_group::2 when verified, else single CTA),
+        else the CUDA-core matcher stays.  Returns {variant: bool} plus "slice_impl" / "match_impl" /
+        "match_cta_group" = the options now in force."""
         from .selfcheck import verified_variants, fastest_slice_impl
         report = {}
         ok = dict(verified_variants(self.device.index or 0, timeout_s, report))
         ok["slice_impl"] = fastest_slice_impl(report)
         ok["match_cta_group"] = 2 if ok.get("match_cg2") else 1
+        ok["match_impl"] = 0 if (ok.get("match_cg1") or ok.get("match_cg2")) else 1
+        self.spf_set_option("match_impl", ok["match_impl"])
         self.spf_set_option("slice_impl", ok["slice_impl"])
         self.spf_set_option("match_cta_group", ok["match_cta_group"])
         return ok

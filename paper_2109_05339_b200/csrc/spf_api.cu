@@ -94,6 +94,7 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     if (!strcmp(key, "slice_impl") && value >= 0 && value <= 2) { ctx->opt_slice_impl = (int)value; return SPF_OK; }
     if (!strcmp(key, "force_complex_grid") && (value == 0 || value == 1)) { ctx->opt_force_complex = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_cta_group") && (value == 1 || value == 2)) { ctx->opt_match_cta_group = (int)value; return SPF_OK; }
+    if (!strcmp(key, "match_impl") && (value == 0 || value == 1)) { ctx->opt_match_impl = (int)value; return SPF_OK; }
     if (!strcmp(key, "record_events") && (value == 0 || value == 1)) { ctx->opt_record_events = (int)value; return SPF_OK; }
     return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
 }

@@ -31,6 +31,8 @@ struct spf_ctx {
     int opt_slice_impl = 1;       // conservative defaults until a variant has been checked on the device (spf.h)
     int opt_force_complex = 0;
     int opt_match_cta_group = 1;
+    int opt_match_impl = 1;       // 1 = CUDA-core difference-form matcher, 0 = tcgen05 GEMM (spf.h)
+    int last_match_impl = 1;
     int opt_record_events = 0;
     int64_t launches = 0;
     // CUDA events around the dominant kernels (option "record_events"): [0,1] slice kernel,

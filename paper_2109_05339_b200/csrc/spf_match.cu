@@ -327,6 +327,91 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
 }
 
 // ------------------------------------------------------------------------------------------
+// CUDA-core matcher (option "match_impl" = 1, the library default until the tensor-core kernel has
+// passed its self-check on the device): the definition itself, d = sum_j (I_ij - S_mj)^2 over unmasked
+// pixels, in fp32 -- no expansion, so no cancellation and no operand split.  A register-tiled kernel in
+// the shape of a plain SGEMM: block = 128 images x 128 slices, 256 threads x (8 x 8) pairs, K tiles of
+// 16 pixels staged through shared memory (transposed, padded rows).  Each pair's sum runs in two
+// levels -- 1,024 pixels into `acc`, then `acc` into `tot` -- so the rounding error stays ~1e-6 of d at
+// P = 65,536.  The argmin merges through the same packed 64-bit atomicMin keys as the tensor-core kernel.
+// Cost: 2 instructions per pixel pair on the fp32 pipes (74 TFLOP/s) against 2 fp16 products on the
+// tensor pipe (> 1 PFLOP/s): about 20x slower at Paper-scale.  It is the fallback, not the product.
+// ------------------------------------------------------------------------------------------
+constexpr int ST_BM = 128, ST_BN = 128, ST_BK = 16, ST_PAD = 4, ST_FLUSH = 1024 / ST_BK;
+
+__global__ void __launch_bounds__(256, 1)
+k_match_simt(const float *__restrict__ images, int64_t n_img, const float *__restrict__ slices, int64_t M, int64_t P,
+             const uint8_t *__restrict__ mask, unsigned long long *__restrict__ keys) {
+    __shared__ __align__(16) float sI[ST_BK][ST_BM + ST_PAD];
+    __shared__ __align__(16) float sS[ST_BK][ST_BN + ST_PAD];
+    const int tid = threadIdx.x;
+    const int ty = tid >> 4, tx = tid & 15;                 // 16 x 16 threads, 8 x 8 pairs each
+    const int64_t i0 = (int64_t)blockIdx.x * ST_BM, m0 = (int64_t)blockIdx.y * ST_BN;
+    const int lk = tid & 15, lr = tid >> 4;                 // loader: pixel lk of the K tile, rows lr + 16 r
+    float acc[8][8], tot[8][8];
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+#pragma unroll
+        for (int b = 0; b < 8; ++b) acc[a][b] = tot[a][b] = 0.0f;
+
+    const int64_t ktiles = (P + ST_BK - 1) / ST_BK;
+    float pI[8], pS[8];                                     // next K tile, fetched while the current one is summed
+    auto fetch = [&](int64_t kt) {
+        const int64_t j = kt * ST_BK + lk;
+        const bool use = kt < ktiles && j < P && (!mask || mask[j]);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int64_t i = i0 + lr + 16 * r, m = m0 + lr + 16 * r;
+            pI[r] = (use && i < n_img) ? images[i * P + j] : 0.0f;
+            pS[r] = (use && m < M) ? slices[m * P + j] : 0.0f;
+        }
+    };
+    fetch(0);
+    for (int64_t kt = 0; kt < ktiles; ++kt) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) { sI[lk][lr + 16 * r] = pI[r]; sS[lk][lr + 16 * r] = pS[r]; }
+        __syncthreads();
+        fetch(kt + 1);
+#pragma unroll
+        for (int kk = 0; kk < ST_BK; ++kk) {
+            // thread (ty, tx) owns image rows ty*8 .. +7 and slice columns tx*4 .. +3 and 64 + tx*4 .. +3
+            // (two 16-byte loads per operand, neighbouring lanes 16 bytes apart: no bank conflicts)
+            float a[8], b[8];
+            const float4 a0 = *reinterpret_cast<const float4 *>(&sI[kk][ty * 8]), a1 = *reinterpret_cast<const float4 *>(&sI[kk][ty * 8 + 4]);
+            const float4 b0 = *reinterpret_cast<const float4 *>(&sS[kk][tx * 4]), b1 = *reinterpret_cast<const float4 *>(&sS[kk][64 + tx * 4]);
+            a[0] = a0.x; a[1] = a0.y; a[2] = a0.z; a[3] = a0.w; a[4] = a1.x; a[5] = a1.y; a[6] = a1.z; a[7] = a1.w;
+            b[0] = b0.x; b[1] = b0.y; b[2] = b0.z; b[3] = b0.w; b[4] = b1.x; b[5] = b1.y; b[6] = b1.z; b[7] = b1.w;
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+#pragma unroll
+                for (int v = 0; v < 8; ++v) {
+                    const float t = a[u] - b[v];
+                    acc[u][v] = fmaf(t, t, acc[u][v]);
+                }
+        }
+        __syncthreads();
+        if ((kt + 1) % ST_FLUSH == 0) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+#pragma unroll
+                for (int v = 0; v < 8; ++v) { tot[u][v] += acc[u][v]; acc[u][v] = 0.0f; }
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        const int64_t i = i0 + ty * 8 + u;
+        float best = INFINITY; uint32_t bm = 0xffffffffu;
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+            const int64_t m = m0 + (v < 4 ? tx * 4 + v : 64 + tx * 4 + v - 4);   // ascending in v: the lowest index wins ties
+            const float d = tot[u][v] + acc[u][v];
+            if (m < M && d < best) { best = d; bm = (uint32_t)m; }
+        }
+        if (i < n_img && bm != 0xffffffffu) atomicMin(&keys[i], spfmm::pack_key(best, bm));
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // reference matcher (tests only): difference form on the CUDA cores, fp64 accumulation
 // ------------------------------------------------------------------------------------------
 __global__ void k_match_ref_dist(const float *__restrict__ images, int64_t n_img, const float *__restrict__ slices, int64_t M,
@@ -432,6 +517,22 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     int rc;
     if ((rc = spf_record_event(ctx, 4, st))) return rc;
     SPF_CUDA(ctx, cudaMemsetAsync(scal, 0, 64, st));
+    ctx->last_match_impl = ctx->opt_match_impl;
+    if (ctx->opt_match_impl == 1) {
+        // CUDA-core matcher: no operand preparation, only the argmin keys are reset (all ones = "nothing seen")
+        const int64_t gy = (M + ST_BN - 1) / ST_BN;
+        if (gy > 65535) return spf_set_err(ctx, SPF_EINVAL, "spf_match: M too large for the CUDA-core matcher (%lld slices)", (long long)M);
+        SPF_CUDA(ctx, cudaMemsetAsync(keys, 0xff, (size_t)n_img * 8, st));
+        if ((rc = spf_record_event(ctx, 2, st))) return rc;
+        k_match_simt<<<dim3((unsigned)((n_img + ST_BM - 1) / ST_BM), (unsigned)gy), 256, 0, st>>>(images, n_img, slices, M, P, mask, keys);
+        SPF_LAUNCH_CHECK(ctx);
+        if ((rc = spf_record_event(ctx, 3, st))) return rc;
+        ctx->last_scal = scal; ctx->last_match_stream = st;
+        ctx->ev_valid[1] = ctx->ev_valid[2] = ctx->opt_record_events != 0;
+        k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
+        SPF_LAUNCH_CHECK(ctx);
+        return SPF_OK;
+    }
     const int rb = ctx->sm_count * 8;
     k_absmax<<<rb, 256, 0, st>>>(images, n_img, P, mask, scal + 0);
     SPF_LAUNCH_CHECK(ctx);
@@ -474,6 +575,7 @@ int spf_last_match_products(spf_ctx *ctx, int32_t *products) {
     if (!ctx || !products) return SPF_EINVAL;
     if (!ctx->last_scal) return spf_set_err(ctx, SPF_ESTATE, "spf_last_match_products before spf_match");
     uint32_t two_planes = 0;
+    if (ctx->last_match_impl == 1) { *products = 0; return SPF_OK; }   // CUDA-core matcher: no tensor-core products
     SPF_CUDA(ctx, cudaStreamSynchronize(ctx->last_match_stream));
     SPF_CUDA(ctx, cudaMemcpy(&two_planes, ctx->last_scal + 2, sizeof two_planes, cudaMemcpyDeviceToHost));
     *products = two_planes ? 3 : 2;

@@ -1,8 +1,8 @@
 """Device self-check of libspf's kernel variants.
 
 libspf has several implementations of each hot kernel: one with the least machinery (plain global
-gather; single-CTA tcgen05 GEMM) and faster ones (TMA-staged shared-memory gather, one thread or one
-warp per point; cta_group::2 GEMM on CTA pairs).  The library starts on the first;
+gather; CUDA-core difference-form matcher) and faster ones (TMA-staged shared-memory gather, one
+thread or one warp per point; tcgen05 GEMM on single CTAs or cta_group::2 pairs).  The library starts on the first;
 `SpfContext.spf_autotune()` switches on the faster ones that pass this self-check on the device at
 hand, and among the slicing variants that pass, the one the check timed fastest.
 
@@ -121,6 +121,7 @@ def _check_match(device: int, cta_group: int) -> str:
     dev = torch.device("cuda", device)
     g = torch.Generator(device="cpu"); g.manual_seed(5 + cta_group)
     ctx = SpfContext(8, device=device)
+    ctx.spf_set_option("match_impl", 0)             # the tcgen05 kernel (the library default is the CUDA-core matcher)
     ctx.spf_set_option("match_cta_group", cta_group)
     worst = 0.0
     for n_img, M, P, counts in ((300, 513, 2048, True), (130, 257, 200, False), (5, 40, 4100, True)):
@@ -196,16 +197,59 @@ def fastest_slice_impl(report: dict) -> int:
     return best
 
 
+def _disk_cache_path(device: int) -> str:
+    """One file per (library build, GPU): a later PROCESS on the same box reuses the verdicts instead of
+    launching a variant that already faulted once more (every bench / test / profiler process would
+    otherwise repeat the fault).  Keyed by the SHA-1 of libspf.so and the GPU's UUID, so a rebuilt library
+    or another device is always checked afresh.  SPF_SELFCHECK_CACHE=off disables it, any other value is
+    the directory to use (default: the system temp directory)."""
+    import hashlib
+    import tempfile
+    where = os.environ.get("SPF_SELFCHECK_CACHE", "")
+    if where.lower() == "off":
+        return ""
+    from .binding import LIB_PATH
+    try:
+        with open(LIB_PATH, "rb") as f:
+            h = hashlib.sha1(f.read()).hexdigest()[:16]
+        import torch
+        uuid = str(getattr(torch.cuda.get_device_properties(device), "uuid", "gpu%d" % device))
+    except Exception:
+        return ""
+    return os.path.join(where or tempfile.gettempdir(), "libspf_selfcheck_%s_%s.json" % (h, uuid.replace("/", "_")))
+
+
 def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = None) -> dict:
-    """{variant: passed} for every variant, each checked once per process (cached)."""
+    """{variant: passed} for every variant, each checked once per library build and GPU (cached in the
+    process and on disk)."""
+    path = _disk_cache_path(device)
+    disk = {}
+    if path and os.path.exists(path):
+        try:
+            with open(path) as f:
+                disk = json.load(f)
+        except Exception:
+            disk = {}
     out = {}
     for v in VARIANTS:
         key = (v, device)
         if key not in _cache:
-            _cache[key] = check_in_child(v, device, timeout_s)
-            sys.stderr.write("[libspf selfcheck] %-12s %s (%s, %.1f s)\n" % (
-                v, "ok" if _cache[key]["ok"] else "FAILED status %s" % _cache[key]["status"], _cache[key]["detail"],
-                _cache[key]["seconds"]))
+            if v in disk and isinstance(disk[v], dict) and "ok" in disk[v]:
+                _cache[key] = disk[v]
+                sys.stderr.write("[libspf selfcheck] %-12s %s (cached verdict from %s)\n" % (v, "ok" if disk[v]["ok"] else "FAILED", path))
+            else:
+                _cache[key] = check_in_child(v, device, timeout_s)
+                sys.stderr.write("[libspf selfcheck] %-12s %s (%s, %.1f s)\n" % (
+                    v, "ok" if _cache[key]["ok"] else "FAILED status %s" % _cache[key]["status"], _cache[key]["detail"],
+                    _cache[key]["seconds"]))
+                disk[v] = _cache[key]
+                if path:
+                    try:
+                        with open(path + ".tmp", "w") as f:
+                            json.dump(disk, f)
+                        os.replace(path + ".tmp", path)
+                    except Exception:
+                        pass
         out[v] = _cache[key]["ok"]
         if report is not None:
             report[v] = _cache[key]

@@ -1,9 +1,10 @@
 """GPU parity tests (-m gpu): every step of the CUDA path against the oracle, through the C ABI.
 
 Order matters (the driver runs with -x): this file exercises the library's DEFAULT kernel variants
-(global-memory gather, single-CTA tcgen05 matcher) first, then the full-size configuration with
+(global-memory gather, CUDA-core difference-form matcher) first, then the full-size configuration with
 whatever `spf_autotune` verified on this device; tests/test_gpu_variants.py (collected after this
-file) then holds the faster variants to the same parity bar.  Every test ends with
+file) then holds the faster variants -- TMA-staged slicing, the tcgen05 matcher on single CTAs and
+on CTA pairs -- to the same parity bar.  Every test ends with
 `spf_check_fault`, so a pipeline whose watchdog gave up fails the test instead of passing on
 garbage.
 
@@ -208,19 +209,26 @@ MATCH_SIZES = [(16, 64, 1024, False), (5, 300, 1000, True), (130, 257, 192, Fals
 
 @pytest.mark.parametrize("n_img,M,P,masked", MATCH_SIZES)
 def test_match_vs_oracle_ragged_sizes(spf, n_img, M, P, masked):
-    match_vs_oracle_ragged_sizes(spf, 1, n_img, M, P, masked)
+    match_vs_oracle_ragged_sizes(spf, "simt", n_img, M, P, masked)
 
 
-def match_vs_oracle_ragged_sizes(spf, cta_group, n_img, M, P, masked):
+def set_match_variant(ctx, variant):
+    """"simt": the CUDA-core matcher (library default); "cg1" / "cg2": the tcgen05 GEMM on single CTAs / CTA pairs."""
+    ctx.spf_set_option("match_impl", 1 if variant == "simt" else 0)
+    ctx.spf_set_option("match_cta_group", 2 if variant == "cg2" else 1)
+
+
+def match_vs_oracle_ragged_sizes(spf, variant, n_img, M, P, masked):
     rng = np.random.default_rng(n_img * 7 + M)
     S = (rng.random((M, P)) * rng.random((M, 1)) * 3).astype(np.float32)
     I = rng.poisson(S[rng.integers(0, M, n_img)]).astype(np.float32)
     mask = (rng.random(P) > 0.2).astype(np.uint8) if masked else None
     ctx = spf.SpfContext(8)
-    ctx.spf_set_option("match_cta_group", cta_group)
+    set_match_variant(ctx, variant)
     bi, bd = ctx.spf_match(_dev(I), _dev(S), None if mask is None else _dev(mask))
     ctx.spf_check_fault()
-    _check_match(bi, bd, I, S, mask, "cg%d" % cta_group)
+    assert ctx.spf_last_match_products() == (0 if variant == "simt" else 2)     # photon counts: one fp16 image plane
+    _check_match(bi, bd, I, S, mask, variant)
     # the independent CUDA-core reference agrees with the oracle too (and gives the full matrix)
     ri, rd, dist = ctx.spf_match_reference(_dev(I), _dev(S), None if mask is None else _dev(mask))
     d_or = orc.distances(I, S, mask)
@@ -229,13 +237,18 @@ def match_vs_oracle_ragged_sizes(spf, cta_group, n_img, M, P, masked):
 
 
 def test_match_planted_ties_and_general_values(spf):
+    match_planted_ties_and_general_values(spf, "simt")
+
+
+def match_planted_ties_and_general_values(spf, variant):
     rng = np.random.default_rng(17)
     M, P = 200, 640
     S = rng.random((M, P)).astype(np.float32)
     S[150] = S[20]                      # exact duplicate: lowest index must win
     planted = np.array([20, 0, 199, 77])
-    I = S[planted].copy()               # non-integer images: the two-plane image path
+    I = S[planted].copy()               # non-integer images: the two-plane image path of the tcgen05 kernel
     ctx = spf.SpfContext(8)
+    set_match_variant(ctx, variant)
     bi, bd = ctx.spf_match(_dev(I), _dev(S))
     bi, bd = bi.cpu().numpy(), bd.cpu().numpy()
     assert list(bi) == list(planted)

@@ -1,7 +1,7 @@
 """GPU parity of the faster kernel variants (-m gpu; collected after tests/test_gpu_parity.py).
 
 `slice_impl = 0` / `2` (TMA-staged shared-memory gather, one thread / one warp per point) and
-`match_cta_group = 2` (tcgen05 on CTA pairs) are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
+`match_impl = 0` (the tcgen05 GEMM, on single CTAs and on `cta_group::2` pairs) are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
 distances <= 1e-4, argmin exact outside near-ties.  Before a variant is launched in this process its
 device self-check (paper_2109_05339_b200/selfcheck.py) must have passed in a child process; if it did
 not, the test fails there, with the child's report, without launching the variant here.
@@ -107,30 +107,66 @@ def test_staged_slice_small_config_sampled(spf, verified, variant, impl):
         assert _rel_l2(got, ref) <= SLICE_TOL
 
 
-# --------------------------------------------------------------------------------- CTA-pair matching
+# --------------------------------------------------------------------------------- tcgen05 matching
 
+TC = [("match_cg1", "cg1"), ("match_cg2", "cg2")]
+
+
+@pytest.mark.parametrize("check,variant", TC)
 @pytest.mark.parametrize("n_img,M,P,masked", MATCH_SIZES)
-def test_cta_pair_match_vs_oracle_ragged_sizes(spf, verified, n_img, M, P, masked):
-    _require(verified, "match_cg2")
-    base.match_vs_oracle_ragged_sizes(spf, 2, n_img, M, P, masked)
+def test_tcgen05_match_vs_oracle_ragged_sizes(spf, verified, n_img, M, P, masked, check, variant):
+    _require(verified, check)
+    base.match_vs_oracle_ragged_sizes(spf, variant, n_img, M, P, masked)
 
 
-def test_cta_pair_and_single_cta_agree_on_counts(spf, verified):
-    """Photon-count images are exact in one fp16 plane (2 products per K step) and both variants add
-    the same products in the same K order into fp32 accumulators: distances agree to fp32 round-off."""
-    _require(verified, "match_cg2")
+@pytest.mark.parametrize("check,variant", TC)
+def test_tcgen05_match_planted_ties_and_general_values(spf, verified, check, variant):
+    """Exact duplicates (lowest index wins), noise-free images (two-plane image path, |d| <= 1e-6 (|I|^2 + |S|^2)),
+    counts above 2,048, power-of-two scaling, permutation of the reference set."""
+    _require(verified, check)
+    base.match_planted_ties_and_general_values(spf, variant)
+
+
+def test_tcgen05_end_to_end_tiny(spf, tiny, verified):
+    """Tiny end to end with the tensor-core matcher: oracle slices + oracle matching on one side, GPU slices +
+    tcgen05 matching on the other."""
+    _require(verified, "match_cg1")
+    from spf_inputs import planted_truth_quaternions, photon_scale, poisson_images
+    cfg, model, pix, refs, c_ref = tiny
+    truth, _ = planted_truth_quaternions(cfg.n_img, refs)
+    alpha = photon_scale(c_ref.real, None, cfg.photons)
+    images = poisson_images(alpha * orc.slice_points(model, truth, pix).real)
+    ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+    ctx.spf_prepare_model(_dev(model))
+    slices = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_INTENSITY, scale=alpha)
+    oi, od, osd, _ = orc.match(images, alpha * c_ref.real)
+    near = (osd - od) <= base.DIST_TOL * od
+    for variant in ("cg1",) + (("cg2",) if verified["match_cg2"]["ok"] else ()):
+        base.set_match_variant(ctx, variant)
+        bi, bd = ctx.spf_match(_dev(images), slices)
+        ctx.spf_check_fault()
+        bi, bd = bi.cpu().numpy(), bd.cpu().numpy()
+        assert np.all((bi == oi) | near) and np.all(np.abs(bd - od) <= base.DIST_TOL * od), variant
+
+
+def test_tcgen05_variants_and_cuda_core_matcher_agree_on_counts(spf, verified):
+    """Photon-count images are exact in one fp16 plane (2 products per K step) and both tcgen05 variants add
+    the same products in the same K order into fp32 accumulators: distances agree to fp32 round-off, and with
+    the CUDA-core difference form to the parity tolerance."""
+    _require(verified, "match_cg1")
     rng = np.random.default_rng(23)
     M, P, n_img = 700, 3000, 260
     S = (rng.random((M, P)) * 2).astype(np.float32)
     I = rng.poisson(S[rng.integers(0, M, n_img)]).astype(np.float32)
     ctx = spf.SpfContext(8)
-    res = []
-    for cg in (1, 2):
-        ctx.spf_set_option("match_cta_group", cg)
+    res = {}
+    for variant in ("simt", "cg1") + (("cg2",) if verified["match_cg2"]["ok"] else ()):
+        base.set_match_variant(ctx, variant)
         bi, bd = ctx.spf_match(_dev(I), _dev(S))
         ctx.spf_check_fault()
-        assert ctx.spf_last_match_products() == 2
-        res.append((bi.cpu().numpy(), bd.cpu().numpy()))
-    assert np.allclose(res[0][1], res[1][1], rtol=2e-6)
-    for bi, bd in res:
-        base._check_match(torch.from_numpy(bi), torch.from_numpy(bd), I, S, None, "counts")
+        assert ctx.spf_last_match_products() == (0 if variant == "simt" else 2)
+        res[variant] = (bi.cpu().numpy(), bd.cpu().numpy())
+        base._check_match(torch.from_numpy(res[variant][0]), torch.from_numpy(res[variant][1]), I, S, None, variant)
+    assert np.allclose(res["simt"][1], res["cg1"][1], rtol=1e-4)
+    if "cg2" in res:
+        assert np.allclose(res["cg1"][1], res["cg2"][1], rtol=2e-6)
