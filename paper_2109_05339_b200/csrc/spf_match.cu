@@ -469,10 +469,7 @@ int launch_gemm(spf_ctx *ctx, const CUtensorMap &a0, const CUtensorMap &a1, cons
     auto kern = k_match_gemm<CG, NI>;
     SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
     const int n_tiles = args.n_ib * args.n_mb;
-    int clusters = ctx->sm_count / CG;
-    if (clusters > n_tiles) clusters = n_tiles;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)(clusters * CG));
     cfg.blockDim = dim3(GEMM_THREADS);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
@@ -480,6 +477,19 @@ int launch_gemm(spf_ctx *ctx, const CUtensorMap &a0, const CUtensorMap &a1, cons
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
+    // Persistent grid with a static tile stride: every cluster must be resident at once, or the ones
+    // that start late run their whole share after the others have finished.  CTA pairs need two free
+    // SMs of one TPC, so fewer than sm_count / 2 pairs may fit: ask the runtime (cached per variant).
+    static int max_clusters = 0;
+    if (max_clusters == 0) {
+        int n = 0;
+        cfg.gridDim = dim3((unsigned)(ctx->sm_count / CG * CG));
+        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) { (void)cudaGetLastError(); n = ctx->sm_count / CG; }
+        max_clusters = n < ctx->sm_count / CG ? n : ctx->sm_count / CG;
+    }
+    int clusters = max_clusters;
+    if (clusters > n_tiles) clusters = n_tiles;
+    cfg.gridDim = dim3((unsigned)(clusters * CG));
     SPF_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, a0, a1, b0, b1, args));
     ctx->launches++;
     return SPF_OK;
