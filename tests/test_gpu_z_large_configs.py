@@ -1,0 +1,99 @@
+"""GPU parity at the two largest configurations (-m gpu; collected last): BASELINE.json:configs[3] Matching-heavy
+and configs[4] Slicing-heavy at their FULL sizes, on sampled outputs the oracle can compute one by one.
+
+They run with whatever `spf_autotune` verified on the device (as bench.py does) and stress what the smaller
+configurations cannot: 64-bit indexing (6.55e9 slice values, 26 GB), 100,000-orientation argmin merges across
+391 slice tiles, the w = 10 kernel (eps = 1e-9; the parity bar stays 1e-5, reading s11) on a 405^3 fine grid.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from spf_inputs import (CONFIGS, make_model, make_detector, make_mask, random_quaternions, photon_scale, poisson_images,
+                        surrogate_slices, sample_pairs)
+
+from test_gpu_parity import spf, _dev, _rel_l2, SLICE_TOL, DIST_TOL  # noqa: F401  (fixture)
+
+pytestmark = [pytest.mark.gpu, pytest.mark.timeout(2400)]
+
+
+def _free_gb():
+    free, _ = torch.cuda.mem_get_info()
+    return free / 2 ** 30
+
+
+def test_slicing_heavy_sampled(spf):
+    """201^3 model, n_fine 405, w = 10; 20,000 orientations x 65,536 pixels = 1.31e9 points sliced on the GPU in two
+    halves of 10,000 orientations (complex output, 5.2 GB each); 2,048 sampled pairs from the oracle."""
+    cfg = CONFIGS["slicing_heavy"]
+    if _free_gb() < 12:
+        pytest.skip("needs 12 GB of free device memory")
+    model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(cfg.M, seed=2)
+    ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+    assert ctx.info.w == 10
+    ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    print("slicing-heavy runs with", ctx.spf_autotune())
+    ctx.spf_prepare_model(_dev(model))
+    assert ctx.info.grid_is_real == 1
+    sm, sj = sample_pairs(cfg.M, cfg.P, 2048)
+    got = np.empty(len(sm), np.complex64)
+    d_pix = _dev(pix)
+    half = cfg.M // 2
+    for lo in (0, half):
+        c = ctx.spf_slice(_dev(refs[lo:lo + half]), d_pix, spf.SPF_OUT_COMPLEX)
+        ctx.spf_check_fault()
+        sel = np.flatnonzero((sm >= lo) & (sm < lo + half))
+        got[sel] = c[torch.from_numpy(sm[sel] - lo).cuda(), torch.from_numpy(sj[sel]).cuda()].cpu().numpy()
+        del c
+    ref = orc.slice_points(model, refs, pix, sm, sj)
+    err = _rel_l2(got, ref)
+    print("slicing-heavy: 2,048 sampled points, relative L2 %.3e" % err)
+    assert err <= SLICE_TOL
+
+
+def test_matching_heavy_sampled(spf):
+    """20,000 Poisson images x 100,000 surrogate slices x 65,536 pixels (5 % masked): 1.3e14 pixel pairs, nothing
+    materialised.  Eight sampled image rows are brute-forced by the oracle against ALL 100,000 slices, ten
+    thousand at a time (the slices do not fit in host memory comfortably as one array)."""
+    cfg = CONFIGS["matching_heavy"]
+    if _free_gb() < 80:
+        pytest.skip("needs 80 GB of free device memory (26 GB slices, 5 GB images, 31 GB operand planes)")
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    mask = make_mask(cfg.panels, cfg.panel_edge, cfg.masked_frac)
+    ctx = spf.SpfContext(8)
+    print("matching-heavy runs with", ctx.spf_autotune())
+    S = torch.empty((cfg.M, cfg.P), dtype=torch.float32, device="cuda")
+    step = 10_000
+    for s in range(0, cfg.M, step):                       # surrogate slices in blocks, each block its own seed
+        S[s:s + step] = surrogate_slices(step, pix, seed=5 + s, device="cuda")
+    alpha = photon_scale(S[:step], mask, cfg.photons)
+    S *= alpha
+    g = torch.Generator(device="cuda"); g.manual_seed(3)
+    truth = torch.randint(0, cfg.M, (cfg.n_img,), generator=g, device="cuda")
+    images = torch.empty((cfg.n_img, cfg.P), dtype=torch.float32, device="cuda")
+    for s in range(0, cfg.n_img, 1000):
+        images[s:s + 1000] = poisson_images(S[truth[s:s + 1000]], seed=4 + s)
+    bi, bd = ctx.spf_match(images, S, _dev(mask))
+    ctx.spf_check_fault()
+    rows = np.random.default_rng(6).choice(cfg.n_img, 8, replace=False)
+    I_h = images[torch.from_numpy(rows).cuda()].cpu().numpy()
+    d = np.empty((len(rows), cfg.M), np.float64)
+    for s in range(0, cfg.M, step):                       # the oracle's distances, block of slices by block
+        d[:, s:s + step] = orc.distances(I_h, S[s:s + step].cpu().numpy(), mask)
+    oi = d.argmin(axis=1)                                 # lowest index on exact ties, as the oracle's own argmin
+    od = d[np.arange(len(rows)), oi]
+    d2 = d.copy()
+    d2[np.arange(len(rows)), oi] = np.inf
+    osd = d2.min(axis=1)
+    gi = bi[torch.from_numpy(rows).cuda()].cpu().numpy()
+    gd = bd[torch.from_numpy(rows).cuda()].cpu().numpy()
+    assert np.all(np.abs(gd - od) <= DIST_TOL * od), "max rel %.3e" % float(np.max(np.abs(gd - od) / od))
+    near = (osd - od) <= DIST_TOL * od
+    assert np.all((gi == oi) | near), (gi, oi)
+    # every image: a valid index and a distance no larger than the one to its own truth slice's neighbourhood
+    assert int(bi.min()) >= 0 and int(bi.max()) < cfg.M and bool(torch.isfinite(bd).all())
+    print("matching-heavy: 8 sampled rows agree with the oracle (%d near-ties), %d images matched their truth slice"
+          % (int(near.sum()), int((bi.long() == truth).sum())))
