@@ -38,7 +38,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
     if failed:
         raise RuntimeError("nvcc failed")
     if procs or force or not os.path.exists(LIB):
-        cmd = [nvcc, "-shared", "-o", LIB + ".tmp", *objs, "-L" + os.path.join(CUDA_HOME, "lib64"), "-lcufft",
+        cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp", *objs, "-L" + os.path.join(CUDA_HOME, "lib64"), "-lcufft",
                "-Xlinker", "-rpath," + os.path.join(CUDA_HOME, "lib64")]
         subprocess.run(cmd, check=True)
         os.replace(LIB + ".tmp", LIB)
