@@ -136,13 +136,18 @@ def _check_match(device: int, cta_group: int) -> str:
             ctx.spf_check_fault()
             ri, rd, dist = ctx.spf_match_reference(dI, dS, dm)
             torch.cuda.synchronize(dev)
+            # tolerance: 1e-4 of d (north_star), or -- where d is a tiny fraction of the norms and the expanded
+            # form cancels in fp32 (the low-noise case below) -- 1e-6 of |I|^2 + |S|^2 (reading s14)
+            keep = torch.ones(P, device=dev) if dm is None else dm.float()
+            nrm = (dI * dI * keep).sum(1) + ((dS * dS * keep).sum(1))[ri.long()]
+            tol = torch.maximum(1e-4 * rd, 1e-6 * nrm)
             rel = ((bd - rd).abs() / rd.clamp_min(1e-30)).max().item()
             worst = max(worst, rel)
-            if not rel <= 1e-4:
+            if not bool(((bd - rd).abs() <= tol).all()):
                 raise AssertionError("cta_group %d: distance differs from the CUDA-core matcher by %.3e" % (cta_group, rel))
             # argmin may differ only where the reference's own margin is within tolerance
             d_at = dist.gather(1, bi.long().clamp(0, M - 1)[:, None])[:, 0]
-            bad = (bi != ri) & ((d_at - rd) > 1e-4 * rd)
+            bad = (bi != ri) & ((d_at - rd) > tol)
             if bool(bad.any()) or bool((bi < 0).any()) or bool((bi >= M).any()):
                 raise AssertionError("cta_group %d: argmin differs from the CUDA-core matcher" % cta_group)
     ctx.close()
