@@ -33,6 +33,7 @@ struct spf_ctx {
     int opt_match_cta_group = 1;
     int opt_match_impl = 1;       // 1 = CUDA-core difference-form matcher, 0 = tcgen05 GEMM (spf.h)
     int last_match_impl = 1;
+    int gemm_max_clusters[2][2] = {{0, 0}, {0, 0}};  // [CG - 1][NI - 1]: co-resident clusters of k_match_gemm, 0 = not asked yet
     int opt_record_events = 0;
     int64_t launches = 0;
     // CUDA events around the dominant kernels (option "record_events"): [0,1] slice kernel,

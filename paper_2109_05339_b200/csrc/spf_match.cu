@@ -479,8 +479,8 @@ int launch_gemm(spf_ctx *ctx, const CUtensorMap &a0, const CUtensorMap &a1, cons
     cfg.attrs = attr; cfg.numAttrs = 1;
     // Persistent grid with a static tile stride: every cluster must be resident at once, or the ones
     // that start late run their whole share after the others have finished.  CTA pairs need two free
-    // SMs of one TPC, so fewer than sm_count / 2 pairs may fit: ask the runtime (cached per variant).
-    static int max_clusters = 0;
+    // SMs of one TPC, so fewer than sm_count / 2 pairs may fit: ask the runtime (cached per context and variant).
+    int &max_clusters = ctx->gemm_max_clusters[CG - 1][NI - 1];
     if (max_clusters == 0) {
         int n = 0;
         cfg.gridDim = dim3((unsigned)(ctx->sm_count / CG * CG));
