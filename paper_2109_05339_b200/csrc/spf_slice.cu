@@ -260,11 +260,13 @@ int build_patches(spf_ctx *ctx, int64_t P) {
 template <int W, bool REAL, int OUTK, int IMPL>
 int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
     auto kern = k_slice<W, REAL, OUTK, IMPL>;
-    // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid
+    // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid (w = 7)
     uint32_t smem = 0;
     args.cap_bytes = 0;
     if (IMPL != IMPL_GLOBAL) {
-        args.cap_bytes = (IMPL == IMPL_COOP ? 48u : 36u) * 1024u * (REAL ? 1u : 2u);
+        // w = 10: an 8 x 16 patch needs up to 73 KB on the real grid (seeded replay of the Slicing-heavy geometry),
+        // 72 KB stages all but a fraction of a percent of the blocks and still leaves three blocks per SM
+        args.cap_bytes = W == 10 ? 72u * 1024u : (IMPL == IMPL_COOP ? 48u : 36u) * 1024u * (REAL ? 1u : 2u);
         smem = args.cap_bytes + (IMPL == IMPL_COOP ? (uint32_t)SPF_COOP_WTS_BYTES : 0u);
         SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         // three (real grid) or two (complex grid) blocks per SM only fit with the largest shared-memory carve-out
