@@ -202,7 +202,7 @@ def _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, quats, pix, table, coo
     quats, pix = np.ascontiguousarray(quats, np.float32), np.ascontiguousarray(pix, np.float32)
     out = np.full((quats.shape[0], pix.shape[0]), np.nan + 0j, np.complex64)
     stats = np.zeros(3, np.int64)
-    cap = (48 if coop else 36) * 1024 * (1 if is_real else 2)        # launch_slice (spf_slice.cu)
+    cap = 72 * 1024 if w == 10 else (48 if coop else 36) * 1024 * (1 if is_real else 2)        # launch_slice (spf_slice.cu)
     sim.hostsim_slice_blocks(grid.ctypes.data, int(is_real), npad, sz, nf, halo, w, quats.ctypes.data, quats.shape[0],
                              pix.ctypes.data, pix.shape[0], table.ctypes.data, len(table) // 128, int(coop), cap,
                              out.ctypes.data, stats.ctypes.data)
@@ -246,6 +246,24 @@ def test_staged_block_replay_ragged_patch_and_complex_general_model(sim):
         c, stats = _slice_blocks(sim, g, 0, npad, sz, nf, halo, w, refs, pix, table, coop)
         assert np.isfinite(c.view(np.float32)).all() and stats[0] > 0
         assert _rel(c, ref) <= SLICE_TOL
+
+
+def test_staged_block_replay_wide_kernel(sim):
+    """w = 10 (eps = 1e-9) through the staged one-thread-per-point path with its 72 KB tile, real and complex grid."""
+    rng = np.random.default_rng(8)
+    N = 21
+    w, nf, halo = _plan(N, 1e-9)
+    assert w == 10
+    pix = make_detector(1, 64)                    # 0.6 fine cells per pixel: an 8 x 16 patch spans about 20 cells
+    refs = random_quaternions(3, seed=31)
+    table = _patch_table(1, 64, 64, 4096)
+    for is_real in (1, 0):
+        A = make_model(N, 12, 5.0) if is_real else rng.standard_normal((N, N, N)).astype(np.float32)
+        g, npad, sz = _padded_grid(sim, A, w, nf, halo)
+        c, stats = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, 0)
+        assert np.isfinite(c.view(np.float32)).all() and stats[0] > 0
+        ref = orc.slice_points(A, refs, pix)
+        assert _rel(c.real if is_real else c, ref.real if is_real else ref) <= SLICE_TOL
 
 
 def test_staged_block_replay_paper_scale_sampled(sim):
