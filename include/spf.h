@@ -135,10 +135,14 @@ SPF_API int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const float *
  * workspace [dev]: at least spf_match_workspace_bytes(n_img, M, P) bytes, 1024-byte aligned.
  *   d_{i,m} = sum_{j: mask_j} (I_ij - S_mj)^2,  best_idx[i] = argmin_m d_{i,m} (lowest m on
  *   exact ties of the computed fp32 distances), best_dist[i] = that distance.
- * Evaluated as ||I||^2 + ||S||^2 - 2 I.S with the cross term on the tensor cores from
- * two-term fp16 splits of both operands (fp32-equivalent products, fp32 accumulation); the
- * distance matrix is never written to memory.  Requires M >= 1 when n_img >= 1.
- * Values must satisfy |x| < 2^100 (they are rescaled by powers of two into fp16 range).
+ * With option match_impl = 0: evaluated as ||I||^2 + ||S||^2 - 2 I.S with the cross term on the
+ * tensor cores from two-term fp16 splits of both operands (fp32-equivalent products, fp32
+ * accumulation); values must satisfy |x| < 2^100 (they are rescaled by powers of two into fp16
+ * range); where d is a tiny fraction of ||I||^2 + ||S||^2 the expansion cancels in fp32 and the
+ * error is bounded by 1e-6 (||I||^2 + ||S||^2) instead of 1e-4 d (reading s14).
+ * With match_impl = 1 (the library's starting value): the sum of squared differences as
+ * written, in fp32 on the CUDA cores.  Either way the distance matrix is never written to
+ * memory.  Requires M >= 1 when n_img >= 1.
  */
 SPF_API int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P,
                       const uint8_t *mask, int32_t *best_idx, float *best_dist, void *workspace,
@@ -147,8 +151,9 @@ SPF_API size_t spf_match_workspace_bytes(int64_t n_img, int64_t M, int64_t P);
 
 /*
  * Debug variant of spf_match for tests: additionally writes the full distance matrix
- * dist [dev] [n_img][M] fp32 with a plain CUDA-core kernel (difference form, fp32) -- used to
- * check the tensor-core path from a second, independent GPU computation.  Small sizes only.
+ * dist [dev] [n_img][M] fp32 with a plain CUDA-core kernel (one block per pair, difference form
+ * accumulated in fp64, rounded once) -- used to check the matchers from a second, independent
+ * GPU computation.  n_img * M < 2^31: small sizes only.
  */
 SPF_API int spf_match_reference(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M,
                                 int64_t P, const uint8_t *mask, int32_t *best_idx, float *best_dist, float *dist,
