@@ -217,7 +217,7 @@ def run_spf(args, cfg):
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
     # kernel variants: the faster ones (TMA-staged gather -- the fastest verified form --, cta_group::2 GEMM) where their device self-check
     # passes in a child process, else the library defaults (paper_2109_05339_b200/selfcheck.py)
-    variants = ({"slice_staged": False, "slice_coop": False, "match_cg1": False, "match_cg2": False, "slice_impl": 1,
+    variants = ({"slice_staged": False, "slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False, "slice_impl": 1,
                  "match_impl": 1, "match_cta_group": 1} if args.no_autotune else ctx.spf_autotune())
     info = ctx.info
     d_model = torch.from_numpy(model).to(dev)
@@ -297,7 +297,7 @@ def run_spf(args, cfg):
                        "n_img_per_gpu": cfg.n_img, "eps": cfg.eps, "masked_frac": cfg.masked_frac,
                        "grid_is_real": bool(info.grid_is_real),
                        "kernel_variants": {"slice": {0: "tma_staged, thread per point", 1: "global_gather, thread per point",
-                                                     2: "tma_staged, warp per point"}[variants["slice_impl"]],
+                                                     2: "tma_staged, warp per point", 3: "global_gather, warp per point"}[variants["slice_impl"]],
                                            "match": ("tcgen05 cta_group::%d" % variants["match_cta_group"]) if variants["match_impl"] == 0
                                                     else "cuda_core difference form (tcgen05 self-check did not pass)",
                                            "selfcheck": variants},

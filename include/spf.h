@@ -184,13 +184,15 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *   "slice_impl":  [1] = plain global-memory gather, one thread per point;
  *                  0 = tile staged in shared memory by TMA, one thread per point gathers from it;
  *                  2 = the same tile, a warp per point: 32 lanes read an 8 x 8 window per x-plane with no
- *                      bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; w = 10 runs as 0)
+ *                      bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; w = 10 runs as 0);
+ *                  3 = the warp-per-point gather straight from global memory (no TMA, mbarrier or tile;
+ *                      w <= 8; w = 10 runs as 1)
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
  *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused norm-add + argmin epilogue (the product);
  *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused
  *                      argmin -- about 20x slower at Paper-scale, no tensor-core, TMA or mbarrier machinery
  *   "match_cta_group": CTAs per tcgen05 MMA (match_impl 0): 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
- * The defaults are the variants with the least machinery; the faster ones (slice_impl 0 / 2, match_impl 0,
+ * The defaults are the variants with the least machinery; the faster ones (slice_impl 0 / 2 / 3, match_impl 0,
  * match_cta_group 2) are switched on by the caller once they have been checked on the device at hand (the Python binding's
  * SpfContext.spf_autotune does that in a child process).
  *   "record_events": [0]; 1 = spf_slice / spf_match record CUDA events on their stream around the

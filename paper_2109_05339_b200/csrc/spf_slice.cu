@@ -59,15 +59,64 @@ __device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t
 //                   rotated lattice is generic), which costs a conflict degree of ~3.5 per load
 //                   (DESIGN.md section 5); the warp-per-point form needs 14 conflict-free loads + 4
 //                   weight loads per point instead of 343 loads / 32 lanes x 3.5.
-enum { IMPL_STAGED = 0, IMPL_GLOBAL = 1, IMPL_COOP = 2 };
+//   IMPL_GCOOP   3  the same warp-per-point walk straight from the grid in global memory: no TMA, no
+//                   mbarrier, no tile -- each load is four 32-byte row segments instead of 32 scattered words
+enum { IMPL_STAGED = 0, IMPL_GLOBAL = 1, IMPL_COOP = 2, IMPL_GCOOP = 3 };
 #define SPF_COOP_WTS_BYTES (SPF_PATCH * SPF_COOP_STRIDE * 4)   // 14,336 = 112 x 128
+
+// The cooperative gather of one warp over its 32 points (variants 2 and 3).  `tile` is the staged box in
+// shared memory (IDX = int, BZ = its row pitch) or the whole padded grid in global memory (IDX = long
+// long, BZ = 0: row pitch `bz` at run time); `cell` is this lane's own point's first cell (< 0: none);
+// `wts_warp` the warp's 32 parked weight sets.  Points go in groups of 8: eight independent gathers in
+// flight per lane, then ONE multi-value butterfly (spf_slice_math.cuh: 4 + 2 + 1 exchanges halve the
+// value count while halving the lane group, 2 more finish) instead of eight 5-step reductions; lane
+// 4 u ends with point u's sum and the owner lanes fetch theirs.
+template <bool REAL, int BZ, typename IDX>
+__device__ __forceinline__ void coop_sweep(const float *tile, IDX cell, int S1, int bz, int w, const float *wts_warp, int lane,
+                                           spfm::c2 &c) {
+    const int h = lane >> 3, k = lane & 7;
+    for (int g0 = 0; g0 < 32; g0 += spfm::MR8) {
+        float pr[spfm::MR8], pi[spfm::MR8];
+#pragma unroll
+        for (int u = 0; u < spfm::MR8; ++u) {
+            const IDX cell_p = __shfl_sync(0xffffffffu, cell, g0 + u);
+            spfm::c2 part; part.x = part.y = 0.0f;
+            if (cell_p >= 0)    // warp-uniform: skips an empty slot of a ragged patch
+                part = spfm::gather_coop_lane<REAL, BZ, IDX>(tile, cell_p, S1, bz, w, wts_warp + (g0 + u) * SPF_COOP_STRIDE, h, k);
+            pr[u] = part.x; pi[u] = part.y;
+        }
+#pragma unroll
+        for (int o = 16, n = spfm::MR8 / 2; n >= 1; o >>= 1, n >>= 1) {
+            const bool upper = (lane & o) != 0;
+#pragma unroll
+            for (int v = 0; v < n; ++v) {
+                const float keep_r = upper ? pr[v + n] : pr[v], send_r = upper ? pr[v] : pr[v + n];
+                pr[v] = keep_r + __shfl_xor_sync(0xffffffffu, send_r, o);
+                if (!REAL) {
+                    const float keep_i = upper ? pi[v + n] : pi[v], send_i = upper ? pi[v] : pi[v + n];
+                    pi[v] = keep_i + __shfl_xor_sync(0xffffffffu, send_i, o);
+                }
+            }
+        }
+#pragma unroll
+        for (int o = 2; o >= 1; o >>= 1) {
+            pr[0] += __shfl_xor_sync(0xffffffffu, pr[0], o);
+            if (!REAL) pi[0] += __shfl_xor_sync(0xffffffffu, pi[0], o);
+        }
+        // the lanes g0 .. g0 + 7 own these points; point u's sum sits in lane mr8_result_lane(u)
+        const float vr = __shfl_sync(0xffffffffu, pr[0], spfm::mr8_result_lane(lane & (spfm::MR8 - 1)));
+        const float vi = REAL ? 0.0f : __shfl_sync(0xffffffffu, pi[0], spfm::mr8_result_lane(lane & (spfm::MR8 - 1)));
+        if ((lane & ~(spfm::MR8 - 1)) == g0) { c.x = vr; c.y = vi; }
+    }
+}
 
 // W = 0: runtime kernel width (any w <= SPF_MAX_W), else compile-time.
 template <int W, bool REAL, int OUTK, int IMPL>
-__global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slice(const __grid_constant__ SliceArgs a) {
-    constexpr bool STAGED = (IMPL != IMPL_GLOBAL);
+__global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMPL_GCOOP) ? 4 : 3) k_slice(const __grid_constant__ SliceArgs a) {
+    constexpr bool STAGED = (IMPL == IMPL_STAGED || IMPL == IMPL_COOP);
     constexpr bool COOP = (IMPL == IMPL_COOP);
-    static_assert(!COOP || (W >= 2 && W <= 8), "the cooperative gather reads an 8 x 8 window per x-plane");
+    constexpr bool GCOOP = (IMPL == IMPL_GCOOP);
+    static_assert(!(COOP || GCOOP) || (W >= 2 && W <= 8), "the cooperative gather reads an 8 x 8 window per x-plane");
     constexpr int WMAX = W ? W : SPF_MAX_W;
     constexpr int E = REAL ? 1 : 2;            // floats per cell
     constexpr int CELL = 4 * E;                // bytes per cell
@@ -82,7 +131,7 @@ __global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slic
     __shared__ uint32_t s_abort;
     extern __shared__ __align__(128) uint8_t s_dyn[];
     // cooperative variant: the first SPF_COOP_WTS_BYTES of dynamic shared memory hold the points' weights
-    uint8_t *s_tile = s_dyn + (COOP ? SPF_COOP_WTS_BYTES : 0);
+    uint8_t *s_tile = s_dyn + ((COOP || GCOOP) ? SPF_COOP_WTS_BYTES : 0);
 
     if (tid == 0) {
         spfm::quat_to_R(a.quats + 4 * m, sR);
@@ -135,7 +184,7 @@ __global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slic
 
     // kernel weights while the tile is in flight
     float wx[WMAX], wy[WMAX], wz[WMAX];
-    if (STAGED) {
+    if (STAGED || GCOOP) {
         spfm::weights_poly<WMAX>(fx, w, a.coef, a.deg, wx); spfm::weights_poly<WMAX>(fy, w, a.coef, a.deg, wy);
         spfm::weights_poly<WMAX>(fz, w, a.coef, a.deg, wz);
     } else {
@@ -145,16 +194,18 @@ __global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slic
 
     spfm::c2 c;
     c.x = c.y = 0.0f;
-    if (STAGED && staged) {
-        if (COOP) {
-            // every lane parks its point's weights where its warp will read them back
-            float pk[24];
-            spfm::coop_pack_weights<WMAX>(pk, w, wx, wy, wz);
-            float4 *dst4 = reinterpret_cast<float4 *>(reinterpret_cast<float *>(s_dyn) + tid * SPF_COOP_STRIDE);
+    const int lane = tid & 31;
+    const float *wts_warp = reinterpret_cast<const float *>(s_dyn) + (tid & ~31) * SPF_COOP_STRIDE;
+    if (COOP || GCOOP) {
+        // every lane parks its point's weights where its warp will read them back
+        float pk[24];
+        spfm::coop_pack_weights<WMAX>(pk, w, wx, wy, wz);
+        float4 *dst4 = reinterpret_cast<float4 *>(reinterpret_cast<float *>(s_dyn) + tid * SPF_COOP_STRIDE);
 #pragma unroll
-            for (int v = 0; v < 6; ++v) dst4[v] = make_float4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
-            __syncwarp();
-        }
+        for (int v = 0; v < 6; ++v) dst4[v] = make_float4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
+        __syncwarp();
+    }
+    if (STAGED && staged) {
         if (!ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort)) {
             if (tid == 0) {
                 a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)patch; a.fault[3] = (uint32_t)(W * 10 + (REAL ? 1 : 0) + 100 * IMPL);
@@ -166,56 +217,24 @@ __global__ void __launch_bounds__(SPF_PATCH, IMPL == IMPL_GLOBAL ? 4 : 3) k_slic
         const float *tile = reinterpret_cast<const float *>(s_tile);
         const int cell = active ? (px - lox) * S1 + (py - loy) * bz + (pz - loz) : -1;
         if (COOP) {
-            const int lane = tid & 31, h = lane >> 3, k = lane & 7;
-            const float *wts_warp = reinterpret_cast<const float *>(s_dyn) + (tid & ~31) * SPF_COOP_STRIDE;
-            // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates.
-            // Points go in groups of 8: eight independent gathers in flight per lane, then ONE multi-value
-            // butterfly (spfm::MR8_*: 4 + 2 + 1 exchanges halve the value count while halving the lane
-            // group, 2 more finish) instead of eight 5-step reductions; lane 4 u ends with point u's sum.
-            auto sweep = [&](auto bz_tag) {
-                constexpr int BZ = decltype(bz_tag)::value;
-                for (int g0 = 0; g0 < 32; g0 += spfm::MR8) {
-                    float pr[spfm::MR8], pi[spfm::MR8];
-#pragma unroll
-                    for (int u = 0; u < spfm::MR8; ++u) {
-                        const int cell_p = __shfl_sync(0xffffffffu, cell, g0 + u);
-                        spfm::c2 part; part.x = part.y = 0.0f;
-                        if (cell_p >= 0)    // warp-uniform: skips an empty slot of a ragged patch
-                            part = spfm::gather_coop_lane<REAL, BZ>(tile, cell_p, S1, bz, w, wts_warp + (g0 + u) * SPF_COOP_STRIDE, h, k);
-                        pr[u] = part.x; pi[u] = part.y;
-                    }
-#pragma unroll
-                    for (int o = 16, n = spfm::MR8 / 2; n >= 1; o >>= 1, n >>= 1) {
-                        const bool upper = (lane & o) != 0;
-#pragma unroll
-                        for (int v = 0; v < n; ++v) {
-                            const float keep_r = upper ? pr[v + n] : pr[v], send_r = upper ? pr[v] : pr[v + n];
-                            pr[v] = keep_r + __shfl_xor_sync(0xffffffffu, send_r, o);
-                            if (!REAL) {
-                                const float keep_i = upper ? pi[v + n] : pi[v], send_i = upper ? pi[v] : pi[v + n];
-                                pi[v] = keep_i + __shfl_xor_sync(0xffffffffu, send_i, o);
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int o = 2; o >= 1; o >>= 1) {
-                        pr[0] += __shfl_xor_sync(0xffffffffu, pr[0], o);
-                        if (!REAL) pi[0] += __shfl_xor_sync(0xffffffffu, pi[0], o);
-                    }
-                    // the lanes g0 .. g0 + 7 own these points; point u's sum sits in lane mr8_result_lane(u)
-                    const float vr = __shfl_sync(0xffffffffu, pr[0], spfm::mr8_result_lane(lane & (spfm::MR8 - 1)));
-                    const float vi = REAL ? 0.0f : __shfl_sync(0xffffffffu, pi[0], spfm::mr8_result_lane(lane & (spfm::MR8 - 1)));
-                    if ((lane & ~(spfm::MR8 - 1)) == g0) { c.x = vr; c.y = vi; }
-                }
-            };
-            if (bz == 24) sweep(std::integral_constant<int, 24>{});
-            else if (bz == 8) sweep(std::integral_constant<int, 8>{});
-            else sweep(std::integral_constant<int, 40>{});
+            // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates
+            if (bz == 24) coop_sweep<REAL, 24, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
+            else if (bz == 8) coop_sweep<REAL, 8, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
+            else coop_sweep<REAL, 40, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
             if (!active) return;
         } else {
             if (!active) return;
             c = spfm::gather<WMAX, REAL>(tile + (size_t)cell * E, S1, bz, w, wx, wy, wz);
         }
+    } else if (COOP || GCOOP) {
+        // the same warp-per-point walk straight from the padded grid (L1/L2): variant 3, and the blocks of
+        // variant 2 whose box does not fit the tile.  The 8 x 8 window reads one row and one cell past the
+        // w taps (weight 0): for finite input the last first-cell is np - 8 (spf_slice_math.cuh), so the
+        // window ends at np - 1; the clamp only acts on the NaN / inf inputs cell_and_fraction parks at np - w.
+        const int qy = min(py, a.np - 8), qz = min(pz, a.np - 8);
+        const long long cell = active ? ((long long)px * a.np + qy) * a.sz + qz : -1;
+        coop_sweep<REAL, 0, long long>(a.grid, cell, a.np * a.sz, a.sz, w, wts_warp, lane, c);
+        if (!active) return;
     } else {
         if (!active) return;
         const float *base = a.grid + ((size_t)((size_t)px * a.np + py) * a.sz + pz) * E;
@@ -263,7 +282,8 @@ int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
     // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid (w = 7)
     uint32_t smem = 0;
     args.cap_bytes = 0;
-    if (IMPL != IMPL_GLOBAL) {
+    if (IMPL == IMPL_GCOOP) smem = (uint32_t)SPF_COOP_WTS_BYTES;   // the parked weights only
+    if (IMPL == IMPL_STAGED || IMPL == IMPL_COOP) {
         // w = 10: an 8 x 16 patch needs up to 73 KB on the real grid (seeded replay of the Slicing-heavy geometry),
         // 72 KB stages all but a fraction of a percent of the blocks and still leaves three blocks per SM
         args.cap_bytes = W == 10 ? 72u * 1024u : (IMPL == IMPL_COOP ? 48u : 36u) * 1024u * (REAL ? 1u : 2u);
@@ -288,10 +308,11 @@ int launch_slice_w(spf_ctx *ctx, SliceArgs &args, int impl, cudaStream_t st) {
     switch (ctx->w) {
         case 7:
             if (impl == IMPL_COOP) return launch_slice<7, REAL, OUTK, IMPL_COOP>(ctx, args, st);
+            if (impl == IMPL_GCOOP) return launch_slice<7, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
             if (impl == IMPL_STAGED) return launch_slice<7, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
             return launch_slice<7, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         case 10:   // 10 x 10 window: the cooperative form (8 x 8) does not apply
-            if (impl != IMPL_GLOBAL) return launch_slice<10, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
+            if (impl == IMPL_STAGED || impl == IMPL_COOP) return launch_slice<10, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
             return launch_slice<10, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         default: return launch_slice<0, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);  // any other width: runtime-w global gather
     }

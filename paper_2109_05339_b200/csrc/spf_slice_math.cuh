@@ -184,13 +184,14 @@ SPF_HD void coop_pack_weights(float (&out)[24], int w, const float (&wx)[WMAX], 
 // box (x-plane pitch S1, row pitch bz), wts = the point's weights as stored above.
 //   sum_t1 wx[t1] (wy[h] wz[k] b[t1][h][k] + wy[h+4] wz[k] b[t1][h+4][k])
 // BZ > 0 fixes the row pitch at compile time (the row offsets become immediates); BZ = 0 uses bz.
-template <bool REAL, int BZ>
-SPF_HD c2 gather_coop_lane(const float *tile, int cell, int S1, int bz, int w, const float *wts, int h, int k) {
+// IDX: int for a shared-memory tile, long long when `tile` is the whole padded grid in global memory.
+template <bool REAL, int BZ, typename IDX = int>
+SPF_HD c2 gather_coop_lane(const float *tile, IDX cell, int S1, int bz, int w, const float *wts, int h, int k) {
     constexpr int E = REAL ? 1 : 2;
     const int rp = BZ ? BZ : bz;
     const float wzk = wts[k];
     const float cA = wts[8 + 2 * h] * wzk, cB = wts[9 + 2 * h] * wzk;
-    const float *p0 = tile + (size_t)(cell + h * rp + k) * E;
+    const float *p0 = tile + (size_t)(cell + (IDX)(h * rp + k)) * E;
     const size_t row4 = (size_t)(4 * rp) * E, plane = (size_t)S1 * E;
     float ar = 0.0f, ai = 0.0f, br = 0.0f, bi = 0.0f;
 #pragma unroll 8

@@ -1,8 +1,8 @@
 """Device self-check of libspf's kernel variants.
 
 libspf has several implementations of each hot kernel: one with the least machinery (plain global
-gather; CUDA-core difference-form matcher) and faster ones (TMA-staged shared-memory gather, one
-thread or one warp per point; tcgen05 GEMM on single CTAs or cta_group::2 pairs).  The library starts on the first;
+gather; CUDA-core difference-form matcher) and faster ones (warp-per-point gather from global memory;
+TMA-staged shared-memory gather, one thread or one warp per point; tcgen05 GEMM on single CTAs or cta_group::2 pairs).  The library starts on the first;
 `SpfContext.spf_autotune()` switches on the faster ones that pass this self-check on the device at
 hand, and among the slicing variants that pass, the one the check timed fastest.
 
@@ -23,8 +23,8 @@ import subprocess
 import sys
 import time
 
-VARIANTS = ("match_cg1", "slice_staged", "slice_coop", "match_cg2")
-SLICE_IMPL = {"slice_staged": 0, "slice_coop": 2}
+VARIANTS = ("match_cg1", "slice_gcoop", "slice_staged", "slice_coop", "match_cg2")
+SLICE_IMPL = {"slice_staged": 0, "slice_coop": 2, "slice_gcoop": 3}
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
 

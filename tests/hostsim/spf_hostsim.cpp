@@ -65,7 +65,8 @@ void hostsim_slice(const float *grid, int is_real, int np, int sz, int nf, int h
 // Replay of one k_slice<STAGED | COOP> launch on the CPU, block by block (spf_slice.cu): patch table ->
 // per-point cell + fraction -> block bounding box -> tile_geom -> the tile image TMA would write (one
 // (by x bz) box per x-plane at pitch S1, zeros outside the padded grid) -> gather from the tile, either
-// one thread per point (coop = 0) or lane by lane as a warp does it (coop = 1: weights parked in the
+// one thread per point (coop = 0) or lane by lane as a warp does it (coop = 1; coop = 2 is variant 3, the same
+// walk with no tile, straight from the grid: weights parked in the
 // 28-float layout, groups of 8 points, partial sums added by the multi-value butterfly).  Everything the tile image
 // does NOT receive from a copy is NaN, so a read outside the staged box poisons the result even
 // where its weight is zero.  stats: [0] blocks staged, [1] blocks not staged (global gather),
@@ -108,7 +109,8 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
         }
         const bool any = hi[0] >= lo[0];
         const int Lx = any ? hi[0] - lo[0] + w : 0, Ly = any ? hi[1] - lo[1] + w : 0, Lz = any ? hi[2] - lo[2] + w : 0;
-        const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, cap_bytes, coop != 0);
+        spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, cap_bytes, coop != 0);
+        if (coop == 2) g.ok = false;        // variant 3: no tile at all
         std::vector<float> tile;
         if (g.ok) {
             n_staged++;
@@ -125,14 +127,29 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
             n_global++;
         }
         spfm::c2 res[PATCH];
-        if (g.ok && coop) {
+        if (coop) {
+            // weights parked in the 28-float layout (slots of empty lanes hold NaN: they must never be read)
             std::vector<float> wts((size_t)PATCH * SPF_COOP_STRIDE, std::nanf(""));
             for (int t = 0; t < PATCH; ++t) {
                 float pk[24];
                 spfm::coop_pack_weights<SPF_MAX_W>(pk, w, wx[t], wy[t], wz[t]);
                 for (int v = 0; v < 24; ++v) wts[(size_t)t * SPF_COOP_STRIDE + v] = jj[t] >= 0 ? pk[v] : std::nanf("");
             }
-            // warp by warp, points in groups of MR8, exactly as k_slice<.., IMPL_COOP> walks them
+            // one lane's partial sum for point t: from the staged tile, or (variant 3, and blocks of variant 2
+            // whose box does not fit) straight from the padded grid with the y / z clamp of the kernel
+            auto lane_part = [&](int t, int lane) {
+                const float *wt = &wts[(size_t)t * SPF_COOP_STRIDE];
+                if (g.ok) {
+                    const int cell = (px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2]);
+                    return is_real ? spfm::gather_coop_lane<true, 0, int>(tile.data(), cell, g.S1, g.bz, w, wt, lane >> 3, lane & 7)
+                                   : spfm::gather_coop_lane<false, 0, int>(tile.data(), cell, g.S1, g.bz, w, wt, lane >> 3, lane & 7);
+                }
+                const int qy = std::min(py[t], np - 8), qz = std::min(pz[t], np - 8);
+                const long long cell = ((long long)px[t] * np + qy) * sz + qz;
+                return is_real ? spfm::gather_coop_lane<true, 0, long long>(grid, cell, np * sz, sz, w, wt, lane >> 3, lane & 7)
+                               : spfm::gather_coop_lane<false, 0, long long>(grid, cell, np * sz, sz, w, wt, lane >> 3, lane & 7);
+            };
+            // warp by warp, points in groups of MR8, exactly as coop_sweep (spf_slice.cu) walks them
             for (int wv = 0; wv < PATCH / 32; ++wv)
                 for (int g0 = 0; g0 < 32; g0 += spfm::MR8) {
                     float pr[32][spfm::MR8], pi[32][spfm::MR8];
@@ -140,11 +157,7 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
                         const int t = wv * 32 + g0 + u;
                         for (int lane = 0; lane < 32; ++lane) {
                             spfm::c2 c; c.x = c.y = 0.0f;
-                            if (jj[t] >= 0) {
-                                const int cell = (px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2]);
-                                c = is_real ? spfm::gather_coop_lane<true, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7)
-                                            : spfm::gather_coop_lane<false, 0>(tile.data(), cell, g.S1, g.bz, w, &wts[(size_t)t * SPF_COOP_STRIDE], lane >> 3, lane & 7);
-                            }
+                            if (jj[t] >= 0) c = lane_part(t, lane);
                             pr[lane][u] = c.x; pi[lane][u] = c.y;
                         }
                     }

@@ -108,3 +108,4 @@ def test_autotune_picks_the_fastest_verified_slicing_variant():
     assert fastest_slice_impl({"slice_staged": ok(2.0), "slice_coop": ok(3.0)}) == 0
     assert fastest_slice_impl({"slice_staged": ok(12.0), "slice_coop": {"ok": False, "metrics": {"slice_ms": 1.0}}}) == 1
     assert fastest_slice_impl({"slice_coop": {"ok": True, "metrics": {}}}) == 1
+    assert fastest_slice_impl({"slice_gcoop": ok(4.0), "slice_coop": ok(6.0), "slice_staged": {"ok": False, "metrics": {}}}) == 3

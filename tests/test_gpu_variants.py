@@ -1,6 +1,7 @@
 """GPU parity of the faster kernel variants (-m gpu; collected after tests/test_gpu_parity.py).
 
-`slice_impl = 0` / `2` (TMA-staged shared-memory gather, one thread / one warp per point) and
+`slice_impl = 3` (warp-per-point gather from global memory), `0` / `2` (TMA-staged shared-memory gather, one
+thread / one warp per point) and
 `match_impl = 0` (the tcgen05 GEMM, on single CTAs and on `cta_group::2` pairs) are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
 distances <= 1e-4, argmin exact outside near-ties.  Before a variant is launched in this process its
 device self-check (paper_2109_05339_b200/selfcheck.py) must have passed in a child process; if it did
@@ -33,14 +34,14 @@ def _require(verified, variant):
         pytest.fail("device self-check of %s did not pass (status %s): %s" % (variant, r["status"], r["detail"]))
 
 
-@pytest.mark.parametrize("variant", ["match_cg1", "slice_staged", "slice_coop", "match_cg2"])
+@pytest.mark.parametrize("variant", ["match_cg1", "slice_gcoop", "slice_staged", "slice_coop", "match_cg2"])
 def test_variant_selfcheck(verified, variant):
     _require(verified, variant)
 
 
 # --------------------------------------------------------------------------------- staged slicing
 
-STAGED = [("slice_staged", 0), ("slice_coop", 2)]
+STAGED = [("slice_gcoop", 3), ("slice_staged", 0), ("slice_coop", 2)]
 
 
 @pytest.mark.parametrize("variant,impl", STAGED)
