@@ -71,18 +71,19 @@ def _check_slice_staged(device: int, impl: int):
 
 
 def _time_slice(device: int, impl: int) -> dict:
-    """Milliseconds of spf_slice for 256 orientations x 16,384 pixels of a 64^3 even model (real grid, w = 7),
-    global gather and variant `impl`, best of 3 (CUDA events on the current stream)."""
+    """Milliseconds of spf_slice for 64 orientations x 65,536 pixels (4 panels of 128 x 128, about 0.9 fine cells
+    per pixel as at Paper-scale) of a 128^3 even model (real grid of 266^3 cells = 75 MB: beyond L1, inside L2,
+    w = 7), global gather and variant `impl`, best of 3 (CUDA events on the current stream)."""
     import torch
     from .binding import SpfContext, SPF_OUT_INTENSITY
     dev = torch.device("cuda", device)
     g = torch.Generator(device="cpu"); g.manual_seed(3)
-    n = 64
+    n = 128
     A = torch.randn((n, n, n), generator=g, dtype=torch.float32)
     idx = (2 * (n // 2) - torch.arange(n)) % n
     A = 0.5 * (A + A[idx][:, idx][:, :, idx])
     A[0] = 0; A[:, 0] = 0; A[:, :, 0] = 0
-    edge = 64
+    edge = 128
     t = (torch.arange(edge, dtype=torch.float64) - (edge - 1) / 2) / (2 * edge)
     pix = []
     for cy in (-0.26, 0.26):
@@ -92,11 +93,12 @@ def _time_slice(device: int, impl: int) -> dict:
             pix.append((k / k.norm(dim=-1, keepdim=True) - torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64)).reshape(-1, 3))
     pix = torch.cat(pix)
     pix = (pix * (0.9 * torch.pi / pix.norm(dim=-1).max())).to(torch.float32).to(dev)
-    quats = torch.randn((256, 4), generator=g, dtype=torch.float32).to(dev)
+    n_or = 64
+    quats = torch.randn((n_or, 4), generator=g, dtype=torch.float32).to(dev)
     ctx = SpfContext(n, eps=1e-6, device=device)
     ctx.spf_set_detector_layout(4, edge, edge)
     ctx.spf_prepare_model(A.to(dev))
-    out = torch.empty((256, pix.shape[0]), dtype=torch.float32, device=dev)
+    out = torch.empty((n_or, pix.shape[0]), dtype=torch.float32, device=dev)
     ms = {}
     for which in (1, impl):
         ctx.spf_set_option("slice_impl", which)
@@ -112,7 +114,7 @@ def _time_slice(device: int, impl: int) -> dict:
         ctx.spf_check_fault()
         ms["global" if which == 1 else "variant"] = best
     ctx.close()
-    return {"slice_ms_global": ms["global"], "slice_ms": ms["variant"], "points": 256 * int(pix.shape[0])}
+    return {"slice_ms_global": ms["global"], "slice_ms": ms["variant"], "points": n_or * int(pix.shape[0])}
 
 
 def _check_match(device: int, cta_group: int) -> str:
