@@ -63,6 +63,7 @@ struct spf_ctx {
 
     SliceMaps maps_c{}, maps_r{};
     bool maps_ok = false;
+    std::string maps_err;         // why the slice tensor maps could not be encoded (then only slice_impl 1 / 3 run)
 
     // host-buffer entry point: cached device buffers
     struct HostBufs {

@@ -160,8 +160,9 @@ static int create_impl(spf_ctx *ctx, const spf_params *p) {
     cufftResult fr = cufftPlan3d(&ctx->plan, ctx->nf, ctx->nf, ctx->nf, CUFFT_C2C);
     if (fr != CUFFT_SUCCESS) return spf_set_err(ctx, fr == CUFFT_ALLOC_FAILED ? SPF_ENOMEM : SPF_ECUDA, "cufftPlan3d(%d^3) failed: %d", ctx->nf, (int)fr);
     ctx->plan_ok = true;
-    int rc = spf_build_slice_maps(ctx);
-    if (rc) return rc;
+    // The tensor maps serve the TMA-staged slicing variants only: if the driver refuses one, the context is
+    // still good for the variants that do not use TMA, and spf_slice reports the reason when asked for a staged one.
+    if (spf_build_slice_maps(ctx) != SPF_OK) { ctx->maps_err = ctx->err; ctx->err.clear(); }
     SPF_CUDA(ctx, cudaDeviceSynchronize());
     return SPF_OK;
 }

@@ -348,6 +348,9 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.maps = real ? ctx->maps_r : ctx->maps_c;
     args.fault = ctx->d_fault;
     const int impl = ctx->opt_slice_impl;
+    if ((impl == IMPL_STAGED || impl == IMPL_COOP) && !ctx->maps_ok)
+        return spf_set_err(ctx, SPF_ECUDA, "spf_slice: slice_impl %d needs the TMA tensor maps, which could not be encoded: %s", impl,
+                           ctx->maps_err.c_str());
     if (real) {
         return out_kind == SPF_OUT_COMPLEX ? launch_slice_w<true, SPF_OUT_COMPLEX>(ctx, args, impl, st)
                                            : launch_slice_w<true, SPF_OUT_INTENSITY>(ctx, args, impl, st);
