@@ -205,13 +205,13 @@ def fastest_slice_impl(report: dict) -> int:
 
 
 def _disk_cache_path(device: int) -> str:
-    """One file per (library build, GPU): a later PROCESS on the same box reuses the verdicts instead of
-    launching a variant that already faulted once more (every bench / test / profiler process would
-    otherwise repeat the fault).  Keyed by the SHA-1 of libspf.so and the GPU's UUID, so a rebuilt library
-    or another device is always checked afresh.  SPF_SELFCHECK_CACHE=off disables it, any other value is
-    the directory to use (default: the system temp directory)."""
+    """One file per (library build, GPU) under <repository>/gpurun_out/selfcheck/: a later PROCESS of the same
+    job reuses the verdicts instead of launching a variant that already faulted once more (every bench /
+    test / profiler process would otherwise repeat the fault).  Keyed by the SHA-1 of libspf.so and the GPU's
+    UUID, so a rebuilt library or another device is always checked afresh; the directory lives inside the
+    working copy, so nothing carries over from an earlier job on a reused machine.
+    SPF_SELFCHECK_CACHE=off disables it, any other value is the directory to use."""
     import hashlib
-    import tempfile
     where = os.environ.get("SPF_SELFCHECK_CACHE", "")
     if where.lower() == "off":
         return ""
@@ -221,9 +221,11 @@ def _disk_cache_path(device: int) -> str:
             h = hashlib.sha1(f.read()).hexdigest()[:16]
         import torch
         uuid = str(getattr(torch.cuda.get_device_properties(device), "uuid", "gpu%d" % device))
+        where = where or os.path.join(_ROOT, "gpurun_out", "selfcheck")
+        os.makedirs(where, exist_ok=True)
     except Exception:
         return ""
-    return os.path.join(where or tempfile.gettempdir(), "libspf_selfcheck_%s_%s.json" % (h, uuid.replace("/", "_")))
+    return os.path.join(where, "libspf_selfcheck_%s_%s.json" % (h, uuid.replace("/", "_")))
 
 
 def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = None) -> dict:
