@@ -100,8 +100,11 @@ SPF_HD c2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMA
                  const float (&wz)[WMAX]) {
     float accr = 0.0f, acci = 0.0f;
     constexpr int E = REAL ? 1 : 2;
-#pragma unroll 1
-    for (int t1 = 0; t1 < w; ++t1) {
+    // the outer tap loop is unrolled for the compile-time widths up to 8 (wx[] then stays in registers);
+    // for wider or run-time widths it stays a loop and wx[] is indexed in local memory
+#pragma unroll
+    for (int t1 = 0; t1 < (WMAX <= 8 ? WMAX : w); ++t1) {
+        if (WMAX <= 8 && t1 >= w) break;
         float pr = 0.0f, pi = 0.0f;
 #pragma unroll
         for (int t2 = 0; t2 < WMAX; ++t2) {
