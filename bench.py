@@ -312,10 +312,13 @@ def run_spf(args, cfg):
             "gpu_launches": int(launches), "planted_hit_rate": hit}
 
     # end to end through the C-ABI host-buffer call (pinned host memory, copies inside the timed region)
-    try:
-        line["e2e"] = run_e2e(args, cfg, ctx, model, refs, pix, mask, images, alpha, world, dist if world > 1 else None)
-    except Exception as e:  # the device-resident number stands on its own
-        line["e2e"] = {"value": None, "unit": UNIT, "error": repr(e)[:200]}
+    if args.no_e2e:
+        line["e2e"] = {"value": None, "unit": UNIT, "skipped": "--no-e2e"}
+    else:
+        try:
+            line["e2e"] = run_e2e(args, cfg, ctx, model, refs, pix, mask, images, alpha, world, dist if world > 1 else None)
+        except Exception as e:  # the device-resident number stands on its own
+            line["e2e"] = {"value": None, "unit": UNIT, "error": repr(e)[:200]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         try:
             base = oracle_sample(cfg, model, pix, mask, refs, ORACLE_POINTS, ORACLE_IMAGES, min(cfg.M, 2000))
@@ -428,6 +431,7 @@ def main():
     ap.add_argument("--impl", default="spf", choices=["spf", "reference"])
     ap.add_argument("--config", default="paper_scale", choices=sorted(CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiler runs)")
     ap.add_argument("--no-autotune", action="store_true", help="library default kernel variants, no device self-check")
     args = ap.parse_args()
     if args.steps < 1:
