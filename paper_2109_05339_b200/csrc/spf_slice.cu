@@ -251,22 +251,9 @@ int build_patches(spf_ctx *ctx, int64_t P) {
     const bool lattice = ctx->lay_panels > 0 && (int64_t)ctx->lay_panels * ctx->lay_rows * ctx->lay_cols == P;
     const int key[3] = {lattice ? ctx->lay_panels : 0, lattice ? ctx->lay_rows : 0, lattice ? ctx->lay_cols : 0};
     if (ctx->d_patch && ctx->patch_P == P && !memcmp(key, ctx->patch_key, sizeof key)) return SPF_OK;
+    static_assert(SPF_PATCH == SPF_PATCH_PIXELS, "block size = pixels per patch");
     std::vector<int32_t> tab;
-    if (lattice) {
-        const int TR = 8, TC = SPF_PATCH / TR;
-        const int R = ctx->lay_rows, C = ctx->lay_cols;
-        for (int p = 0; p < ctx->lay_panels; ++p)
-            for (int r0 = 0; r0 < R; r0 += TR)
-                for (int c0 = 0; c0 < C; c0 += TC)
-                    for (int t = 0; t < SPF_PATCH; ++t) {
-                        const int r = r0 + t / TC, c = c0 + t % TC;
-                        tab.push_back((r < R && c < C) ? (int32_t)(((int64_t)p * R + r) * C + c) : -1);
-                    }
-    } else {
-        const int64_t n = (P + SPF_PATCH - 1) / SPF_PATCH;
-        tab.resize((size_t)n * SPF_PATCH);
-        for (int64_t i = 0; i < n * SPF_PATCH; ++i) tab[(size_t)i] = i < P ? (int32_t)i : -1;
-    }
+    spfm::build_patch_table(key[0], key[1], key[2], P, tab);
     if (ctx->d_patch) { cudaFree(ctx->d_patch); ctx->d_patch = nullptr; }
     SPF_CUDA(ctx, cudaMalloc(&ctx->d_patch, tab.size() * sizeof(int32_t)));
     SPF_CUDA(ctx, cudaMemcpy(ctx->d_patch, tab.data(), tab.size() * sizeof(int32_t), cudaMemcpyHostToDevice));

@@ -228,6 +228,29 @@ SPF_HD int mr8_result_lane(int u) { return u << 2; }   // a lane that ends with 
 // ------------------------------------------------------------------------------------------
 // host side (fp64): kernel, polynomial fit of the weights, deapodisation factors
 // ------------------------------------------------------------------------------------------
+// pixel -> patch table of spf_slice: SPF_PATCH_PIXELS pixels per thread block.  Under a detector layout promise
+// (panels x rows x cols == P) a patch is an 8 x 16 lattice tile of one panel (ragged tiles at the panel edges
+// are padded with -1); otherwise patches are runs of consecutive pixels.  Every pixel appears exactly once.
+#define SPF_PATCH_PIXELS 128
+inline void build_patch_table(int panels, int rows, int cols, int64_t P, std::vector<int32_t> &tab) {
+    tab.clear();
+    const bool lattice = panels > 0 && rows > 0 && cols > 0 && (int64_t)panels * rows * cols == P;
+    if (lattice) {
+        const int TR = 8, TC = SPF_PATCH_PIXELS / TR;
+        for (int p = 0; p < panels; ++p)
+            for (int r0 = 0; r0 < rows; r0 += TR)
+                for (int c0 = 0; c0 < cols; c0 += TC)
+                    for (int t = 0; t < SPF_PATCH_PIXELS; ++t) {
+                        const int r = r0 + t / TC, c = c0 + t % TC;
+                        tab.push_back((r < rows && c < cols) ? (int32_t)(((int64_t)p * rows + r) * cols + c) : -1);
+                    }
+    } else {
+        const int64_t n = (P + SPF_PATCH_PIXELS - 1) / SPF_PATCH_PIXELS;
+        tab.resize((size_t)n * SPF_PATCH_PIXELS);
+        for (int64_t i = 0; i < n * SPF_PATCH_PIXELS; ++i) tab[(size_t)i] = i < P ? (int32_t)i : -1;
+    }
+}
+
 inline double es_phi(double z, double beta) { return fabs(z) <= 1.0 ? exp(beta * (sqrt(1.0 - z * z) - 1.0)) : 0.0; }
 
 // Per-tap Chebyshev interpolants of phi on the fraction interval, converted to monomials in u.

@@ -204,6 +204,15 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
     stats[0] = n_staged; stats[1] = n_global; stats[2] = max_tile;
 }
 
+// the patch table spf_slice builds (spf_slice_math.cuh); returns the number of entries, fills out if it is large enough
+long hostsim_patch_table(int panels, int rows, int cols, long P, int *out, long cap) {
+    std::vector<int32_t> tab;
+    spfm::build_patch_table(panels, rows, cols, P, tab);
+    if ((long)tab.size() <= cap)
+        for (size_t i = 0; i < tab.size(); ++i) out[i] = tab[i];
+    return (long)tab.size();
+}
+
 // tile geometry alone, for the menu / capacity tests
 void hostsim_tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, unsigned cap, int coop, int *out4) {
     const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, cell_bytes, cap, coop != 0);

@@ -37,6 +37,8 @@ def sim():
     L.hostsim_slice_blocks.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_long,
                                        C.c_void_p, C.c_long, C.c_void_p, C.c_long, C.c_int, C.c_uint, C.c_void_p, C.c_void_p]
     L.hostsim_tile_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_int, C.c_void_p]
+    L.hostsim_patch_table.argtypes = [C.c_int, C.c_int, C.c_int, C.c_long, C.c_void_p, C.c_long]
+    L.hostsim_patch_table.restype = C.c_long
     return L
 
 
@@ -181,20 +183,32 @@ def test_paper_scale_sampled_vs_oracle(sim):
 # ------------------------------------------------------------------------------------------------
 # staged kernels (slice_impl 0 and 2): block-level replay of the tile staging and of the warp-per-point gather
 # ------------------------------------------------------------------------------------------------
-def _patch_table(panels, rows, cols, P):
-    """build_patches (spf_slice.cu): 8 x 16 lattice tiles per panel under a layout promise, else runs of 128."""
-    tab = []
-    if panels:
-        for p in range(panels):
-            for r0 in range(0, rows, 8):
-                for c0 in range(0, cols, 16):
-                    for t in range(128):
-                        r, c = r0 + t // 16, c0 + t % 16
-                        tab.append((p * rows + r) * cols + c if (r < rows and c < cols) else -1)
-    else:
-        n = (P + 127) // 128
-        tab = [i if i < P else -1 for i in range(n * 128)]
-    return np.asarray(tab, np.int32)
+def _patch_table(sim, panels, rows, cols, P):
+    """The table spf_slice itself builds (build_patch_table, spf_slice_math.cuh), through the host-compiled header."""
+    n = sim.hostsim_patch_table(panels, rows, cols, P, None, 0)
+    tab = np.empty(n, np.int32)
+    assert sim.hostsim_patch_table(panels, rows, cols, P, tab.ctypes.data, n) == n
+    return tab
+
+
+def test_patch_table_covers_every_pixel_once(sim):
+    """Lattice layout: 8 x 16 tiles of one panel, ragged panel edges padded with -1; no promise (or a promise that
+    does not multiply out to P): runs of 128 consecutive pixels.  Every pixel index appears exactly once."""
+    for panels, rows, cols, P in ((1, 32, 32, 1024), (4, 128, 128, 65536), (1, 40, 40, 1600), (3, 9, 17, 459),
+                                  (0, 0, 0, 777), (2, 16, 16, 500), (0, 0, 0, 128), (1, 1, 1, 1)):
+        tab = _patch_table(sim, panels, rows, cols, P)
+        assert len(tab) % 128 == 0
+        real = tab[tab >= 0]
+        assert len(real) == P and np.array_equal(np.sort(real), np.arange(P))
+        lattice = panels > 0 and panels * rows * cols == P
+        if lattice:
+            assert len(tab) == panels * -(-rows // 8) * -(-cols // 16) * 128
+            first = tab[:128].reshape(8, 16)                   # first tile of panel 0: rows 0..7 x cols 0..15
+            rr, cc = np.meshgrid(np.arange(8), np.arange(16), indexing="ij")
+            want = np.where((rr < rows) & (cc < cols), rr * cols + cc, -1)
+            assert np.array_equal(first, want)
+        else:
+            assert len(tab) == -(-P // 128) * 128 and np.array_equal(tab[:P], np.arange(P))
 
 
 def _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, quats, pix, table, coop, cap=None):
@@ -222,7 +236,7 @@ def test_staged_block_replay_tiny_full_vs_oracle(sim, coop, is_real, layout):
     refs = random_quaternions(cfg.M, seed=2)
     w, nf, halo = _plan(cfg.N, cfg.eps)
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
-    table = _patch_table(1, 32, 32, cfg.P) if layout else _patch_table(0, 0, 0, cfg.P)
+    table = _patch_table(sim, 1, 32, 32, cfg.P) if layout else _patch_table(sim, 0, 0, 0, cfg.P)
     c, stats = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, coop)
     assert np.isfinite(c.view(np.float32)).all()
     assert (stats[0] > 0 or coop == 2) and stats[0] + stats[1] == cfg.M * (len(table) // 128)
@@ -244,7 +258,7 @@ def test_staged_block_replay_ragged_patch_and_complex_general_model(sim):
     refs = random_quaternions(5, seed=31)
     w, nf, halo = _plan(N, 1e-6)
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
-    table = _patch_table(0, 0, 0, 200)
+    table = _patch_table(sim, 0, 0, 0, 200)
     ref = orc.slice_points(A, refs, pix)
     for coop in (0, 1):
         c, stats = _slice_blocks(sim, g, 0, npad, sz, nf, halo, w, refs, pix, table, coop)
@@ -261,7 +275,7 @@ def test_warp_per_point_fallback_blocks_equal_the_staged_ones(sim):
     refs = random_quaternions(8, seed=2)
     w, nf, halo = _plan(cfg.N, cfg.eps)
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
-    table = _patch_table(1, 32, 32, cfg.P)
+    table = _patch_table(sim, 1, 32, 32, cfg.P)
     for is_real in (1, 0):
         staged, st1 = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, 1)
         forced, st2 = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, 1, cap=1024)
@@ -278,7 +292,7 @@ def test_staged_block_replay_wide_kernel(sim):
     assert w == 10
     pix = make_detector(1, 64)                    # 0.6 fine cells per pixel: an 8 x 16 patch spans about 20 cells
     refs = random_quaternions(3, seed=31)
-    table = _patch_table(1, 64, 64, 4096)
+    table = _patch_table(sim, 1, 64, 64, 4096)
     for is_real in (1, 0):
         A = make_model(N, 12, 5.0) if is_real else rng.standard_normal((N, N, N)).astype(np.float32)
         g, npad, sz = _padded_grid(sim, A, w, nf, halo)
@@ -297,7 +311,7 @@ def test_staged_block_replay_paper_scale_sampled(sim):
     refs = random_quaternions(4, seed=2)
     w, nf, halo = _plan(cfg.N, cfg.eps)
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
-    table = _patch_table(cfg.panels, cfg.panel_edge, cfg.panel_edge, cfg.P)
+    table = _patch_table(sim, cfg.panels, cfg.panel_edge, cfg.panel_edge, cfg.P)
     c, stats = _slice_blocks(sim, g, 1, npad, sz, nf, halo, w, refs, pix, table, 1)
     assert stats[1] == 0 and stats[2] <= 48 * 1024, stats
     assert np.isfinite(c.view(np.float32)).all()
