@@ -36,12 +36,10 @@ __global__ void k_check_even(const float *__restrict__ A, int N, int *__restrict
 __global__ void k_deapod_pad(const float *__restrict__ A, const float *__restrict__ p, int N, int nf,
                              float2 *__restrict__ fine) {
     const size_t total = (size_t)N * N * N;
-    const int c = N / 2;
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         int i3 = (int)(idx % N), i2 = (int)((idx / N) % N), i1 = (int)(idx / ((size_t)N * N));
-        int l1 = i1 - c, l2 = i2 - c, l3 = i3 - c;
-        l1 += (l1 < 0) ? nf : 0; l2 += (l2 < 0) ? nf : 0; l3 += (l3 < 0) ? nf : 0;
-        float v = A[idx] * (p[i1] * p[i2]) * p[i3];
+        const int l1 = spfm::fine_index_of_voxel(i1, N, nf), l2 = spfm::fine_index_of_voxel(i2, N, nf), l3 = spfm::fine_index_of_voxel(i3, N, nf);
+        const float v = spfm::deapodised(A[idx], p[i1], p[i2], p[i3]);
         fine[((size_t)l1 * nf + l2) * nf + l3] = make_float2(v, 0.0f);
     }
 }
@@ -55,8 +53,7 @@ __global__ void k_relayout(const float2 *__restrict__ fine, int nf, int np, int 
         int pz = (int)(idx % sz), py = (int)((idx / sz) % np), px = (int)(idx / ((size_t)sz * np));
         float2 v = make_float2(0.f, 0.f);
         if (pz < np) {
-            int l1 = (px - off) % nf, l2 = (py - off) % nf, l3 = (pz - off) % nf;
-            l1 += (l1 < 0) ? nf : 0; l2 += (l2 < 0) ? nf : 0; l3 += (l3 < 0) ? nf : 0;
+            const int l1 = spfm::fine_index_of_padded(px, off, nf), l2 = spfm::fine_index_of_padded(py, off, nf), l3 = spfm::fine_index_of_padded(pz, off, nf);
             v = fine[((size_t)l1 * nf + l2) * nf + l3];
         }
         gc[idx] = v;

@@ -38,6 +38,21 @@ namespace spfm {
 
 struct alignas(8) c2 { float x, y; };
 
+// Index maps of spf_prepare_model (steps a1-a2), shared by the kernels and the CPU replay:
+//   model voxel index i (0..N-1), n = i - floor(N/2)      ->  fine-grid index n mod n_f          (deapodise + pad)
+//   padded index p of the centred grid with its periodic halo ->  fine-grid index (p - off) mod n_f (relayout),
+//   off = n_f/2 + halo, so padded index p holds fine cell l = p - off, l in [-off, n_f/2 + halo)
+SPF_HD int fine_index_of_voxel(int i, int N, int nf) {
+    const int l = i - N / 2;
+    return l < 0 ? l + nf : l;
+}
+SPF_HD int fine_index_of_padded(int p, int off, int nf) {
+    const int l = (p - off) % nf;
+    return l < 0 ? l + nf : l;
+}
+// deapodised value of one voxel, in the kernel's operand order (fp32)
+SPF_HD float deapodised(float a, float p1, float p2, float p3) { return a * (p1 * p2) * p3; }
+
 // rotation matrix of the normalised quaternion, fp64 (reading s2: (w,x,y,z), Hamilton, active)
 SPF_HD void quat_to_R(const float *q4, double *R) {
     double w = q4[0], x = q4[1], y = q4[2], z = q4[3];

@@ -213,6 +213,35 @@ long hostsim_patch_table(int panels, int rows, int cols, long P, int *out, long 
     return (long)tab.size();
 }
 
+// spf_prepare_model's two index kernels replayed with the header's maps: k_deapod_pad (model -> zeroed fine grid,
+// complex64 interleaved) and k_relayout (fine grid after the FFT -> centred padded grid [np][np][sz], zeros in the
+// z padding beyond np)
+void hostsim_scatter_model(const float *A, const float *p32, int N, int nf, float *fine /*[nf^3][2], zeroed*/) {
+    for (int i1 = 0; i1 < N; ++i1)
+        for (int i2 = 0; i2 < N; ++i2)
+            for (int i3 = 0; i3 < N; ++i3) {
+                const size_t l = ((size_t)spfm::fine_index_of_voxel(i1, N, nf) * nf + spfm::fine_index_of_voxel(i2, N, nf)) * nf +
+                                 spfm::fine_index_of_voxel(i3, N, nf);
+                fine[2 * l] = spfm::deapodised(A[((size_t)i1 * N + i2) * N + i3], p32[i1], p32[i2], p32[i3]);
+                fine[2 * l + 1] = 0.0f;
+            }
+}
+void hostsim_relayout(const float *fine /*[nf^3][2]*/, int nf, int np, int sz, int off, float *gc /*[np][np][sz][2]*/) {
+#pragma omp parallel for schedule(static)
+    for (int px = 0; px < np; ++px)
+        for (int py = 0; py < np; ++py)
+            for (int pz = 0; pz < sz; ++pz) {
+                const size_t o = ((size_t)px * np + py) * sz + pz;
+                float re = 0.0f, im = 0.0f;
+                if (pz < np) {
+                    const size_t l = ((size_t)spfm::fine_index_of_padded(px, off, nf) * nf + spfm::fine_index_of_padded(py, off, nf)) * nf +
+                                     spfm::fine_index_of_padded(pz, off, nf);
+                    re = fine[2 * l]; im = fine[2 * l + 1];
+                }
+                gc[2 * o] = re; gc[2 * o + 1] = im;
+            }
+}
+
 // tile geometry alone, for the menu / capacity tests
 void hostsim_tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, unsigned cap, int coop, int *out4) {
     const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, cell_bytes, cap, coop != 0);

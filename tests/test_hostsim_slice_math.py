@@ -37,6 +37,8 @@ def sim():
     L.hostsim_slice_blocks.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_long,
                                        C.c_void_p, C.c_long, C.c_void_p, C.c_long, C.c_int, C.c_uint, C.c_void_p, C.c_void_p]
     L.hostsim_tile_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_int, C.c_void_p]
+    L.hostsim_scatter_model.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+    L.hostsim_relayout.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
     L.hostsim_patch_table.argtypes = [C.c_int, C.c_int, C.c_int, C.c_long, C.c_void_p, C.c_long]
     L.hostsim_patch_table.restype = C.c_long
     return L
@@ -58,22 +60,27 @@ def _plan(N, eps):
 
 
 def _padded_grid(sim, A, w, nf, halo):
-    """spf_prepare_model in NumPy: deapodise (fp32, the kernel's operand order), scatter at n mod n_f,
-    forward FFT, centred layout with periodic halo (padded index p <-> fine cell (p - off) mod n_f)."""
+    """spf_prepare_model on the CPU: deapodise + scatter (k_deapod_pad) and the centred layout with periodic halo
+    (k_relayout) through the header's own index maps, host-compiled; the forward FFT in between is NumPy's, in
+    fp64, stored as complex64 (cuFFT's fp32 rounding is what this replay does not see)."""
     N = A.shape[0]
     p = np.empty(N)
     sim.hostsim_deapod(N, nf, w, p.ctypes.data)
     p32 = p.astype(np.float32)
-    v = (A * (p32[:, None, None] * p32[None, :, None])) * p32[None, None, :]
     fine = np.zeros((nf, nf, nf), np.complex64)
+    sim.hostsim_scatter_model(np.ascontiguousarray(A, np.float32).ctypes.data, p32.ctypes.data, N, nf, fine.ctypes.data)
+    # independent restatement of the scatter (deapodised model at index n mod n_f): the two must agree exactly
     idx = (np.arange(N) - N // 2) % nf
-    fine[np.ix_(idx, idx, idx)] = v
-    b = np.fft.fftn(fine.astype(np.complex128)).astype(np.complex64)
+    want = np.zeros((nf, nf, nf), np.complex64)
+    want[np.ix_(idx, idx, idx)] = (A * (p32[:, None, None] * p32[None, :, None])) * p32[None, None, :]
+    assert np.array_equal(fine, want)
+    b = np.ascontiguousarray(np.fft.fftn(fine.astype(np.complex128)).astype(np.complex64))
     npad = nf + 2 * halo
     sz = (npad + 3) & ~3
+    g = np.empty((npad, npad, sz), np.complex64)
+    sim.hostsim_relayout(b.ctypes.data, nf, npad, sz, nf // 2 + halo, g.ctypes.data)
     l = (np.arange(npad) - (nf // 2 + halo)) % nf
-    g = np.zeros((npad, npad, sz), np.complex64)
-    g[:, :, :npad] = b[np.ix_(l, l, l)]
+    assert np.array_equal(g[:, :, :npad], b[np.ix_(l, l, l)]) and not g[:, :, npad:].any()
     return g, npad, sz
 
 
