@@ -19,14 +19,10 @@
 // index-0 planes must be exactly zero for the fine grid to be real.
 __global__ void k_check_even(const float *__restrict__ A, int N, int *__restrict__ bad) {
     const size_t total = (size_t)N * N * N;
-    const int c2 = 2 * (N / 2);
     int local = 0;
     for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         int i3 = (int)(idx % N), i2 = (int)((idx / N) % N), i1 = (int)(idx / ((size_t)N * N));
-        int j1 = c2 - i1, j2 = c2 - i2, j3 = c2 - i3;
-        float a = A[idx];
-        if (j1 >= N || j2 >= N || j3 >= N) local += (a != 0.0f);
-        else local += (a != A[((size_t)j1 * N + j2) * N + j3]);
+        local += spfm::voxel_breaks_evenness(A, N, i1, i2, i3) ? 1 : 0;
     }
     local = __reduce_add_sync(0xffffffffu, local);
     if ((threadIdx.x & 31) == 0 && local) atomicAdd(bad, local);

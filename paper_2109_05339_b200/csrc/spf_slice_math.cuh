@@ -50,6 +50,15 @@ SPF_HD int fine_index_of_padded(int p, int off, int nf) {
     const int l = (p - off) % nf;
     return l < 0 ? l + nf : l;
 }
+// Evenness test of the model (k_check_even): the voxel at -n has index 2 floor(N/2) - i; for even N the
+// index-0 planes have no partner (the result is N) and must be exactly zero for the fine grid to be real.
+SPF_HD int mirror_voxel(int i, int N) { return 2 * (N / 2) - i; }
+SPF_HD bool voxel_breaks_evenness(const float *A, int N, int i1, int i2, int i3) {
+    const int j1 = mirror_voxel(i1, N), j2 = mirror_voxel(i2, N), j3 = mirror_voxel(i3, N);
+    const float a = A[((size_t)i1 * N + i2) * N + i3];
+    if (j1 >= N || j2 >= N || j3 >= N) return a != 0.0f;
+    return a != A[((size_t)j1 * N + j2) * N + j3];
+}
 // deapodised value of one voxel, in the kernel's operand order (fp32)
 SPF_HD float deapodised(float a, float p1, float p2, float p3) { return a * (p1 * p2) * p3; }
 

@@ -242,6 +242,15 @@ void hostsim_relayout(const float *fine /*[nf^3][2]*/, int nf, int np, int sz, i
             }
 }
 
+// k_check_even replayed: number of voxels that break A[n] == A[-n]
+long hostsim_count_uneven(const float *A, int N) {
+    long bad = 0;
+    for (int i1 = 0; i1 < N; ++i1)
+        for (int i2 = 0; i2 < N; ++i2)
+            for (int i3 = 0; i3 < N; ++i3) bad += spfm::voxel_breaks_evenness(A, N, i1, i2, i3) ? 1 : 0;
+    return bad;
+}
+
 // tile geometry alone, for the menu / capacity tests
 void hostsim_tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, unsigned cap, int coop, int *out4) {
     const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, cell_bytes, cap, coop != 0);

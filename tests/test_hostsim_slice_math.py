@@ -39,6 +39,8 @@ def sim():
     L.hostsim_tile_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_int, C.c_void_p]
     L.hostsim_scatter_model.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]
     L.hostsim_relayout.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    L.hostsim_count_uneven.argtypes = [C.c_void_p, C.c_int]
+    L.hostsim_count_uneven.restype = C.c_long
     L.hostsim_patch_table.argtypes = [C.c_int, C.c_int, C.c_int, C.c_long, C.c_void_p, C.c_long]
     L.hostsim_patch_table.restype = C.c_long
     return L
@@ -95,6 +97,28 @@ def _slice(sim, g, is_real, npad, sz, nf, halo, w, quats, pix, use_poly):
 
 def _rel(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def test_evenness_check_decides_when_the_fine_grid_is_real(sim):
+    """k_check_even's rule (replayed): zero voxels break A[n] == A[-n] exactly when the transform of the model is
+    real -- odd N: plain point symmetry about the centre voxel; even N: the unpaired index-0 planes must be zero."""
+    rng = np.random.default_rng(2)
+    count = lambda A: sim.hostsim_count_uneven(np.ascontiguousarray(A, np.float32).ctypes.data, A.shape[0])
+    imag_frac = lambda A: (lambda F: float(np.abs(F.imag).max() / np.abs(F.real).max()))(
+        np.fft.fftn(np.roll(A.astype(np.float64), [-(A.shape[0] // 2)] * 3, (0, 1, 2))))
+    tiny = CONFIGS["tiny"]
+    A = make_model(tiny.N, tiny.n_atoms, tiny.atom_radius)
+    assert count(A) == 0 and imag_frac(A) < 1e-12
+    B = A.copy(); B[3, 4, 5] += 1e-3
+    assert count(B) == 2 and imag_frac(B) > 1e-6               # the voxel and its partner
+    for N in (8, 12):
+        R = rng.standard_normal((N, N, N)).astype(np.float32)
+        idx = (N - np.arange(N)) % N                            # mirror about index N/2: i -> N - i (index 0 maps to itself)
+        S = (0.5 * (R + R[np.ix_(idx, idx, idx)])).astype(np.float32)
+        assert count(S) > 0                                     # index-0 planes are not zero: unpaired frequencies
+        S[0] = 0; S[:, 0] = 0; S[:, :, 0] = 0
+        assert count(S) == 0 and imag_frac(S) < 1e-6
+        assert count(R) > 0
 
 
 def test_polynomial_weights_reach_1e7(sim):
