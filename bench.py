@@ -252,25 +252,37 @@ def run_spf(args, cfg):
         step()
     ctx.spf_check_fault()      # raises if any kernel's watchdog gave up: no number from a broken pipeline
     products = ctx.spf_last_match_products() if args.warmup > 0 else None
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-    k_ms = {"slice": [], "gemm": [], "match_prep": []}
-    sync_all()
-    launches0 = ctx.spf_launch_count()
-    with ClockSampler(physical_gpu_index(local)) as clocks:
-        for k in range(args.steps):
-            ev[k][0].record()
-            ctx.spf_prepare_model(d_model)
-            ev[k][1].record()
-            ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=alpha, out=slices)
-            ev[k][2].record()
-            best_idx, best_dist = ctx.spf_match(images, slices, d_mask)
-            ev[k][3].record()
-            k_ms["slice"].append(ctx.spf_last_kernel_ms(0))       # these synchronise on the library's own events
-            k_ms["gemm"].append(ctx.spf_last_kernel_ms(1))
-            k_ms["match_prep"].append(ctx.spf_last_kernel_ms(2))
+    def measure():
+        """EXACTLY args.steps timed steps between two barriers; CUDA events on the current stream; clocks sampled."""
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+        k_ms = {"slice": [], "gemm": [], "match_prep": []}
         sync_all()
-    ctx.spf_check_fault()
-    launches = ctx.spf_launch_count() - launches0
+        launches0 = ctx.spf_launch_count()
+        with ClockSampler(physical_gpu_index(local)) as clocks:
+            for k in range(args.steps):
+                ev[k][0].record()
+                ctx.spf_prepare_model(d_model)
+                ev[k][1].record()
+                ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=alpha, out=slices)
+                ev[k][2].record()
+                bi, bd = ctx.spf_match(images, slices, d_mask)
+                ev[k][3].record()
+                k_ms["slice"].append(ctx.spf_last_kernel_ms(0))       # these synchronise on the library's own events
+                k_ms["gemm"].append(ctx.spf_last_kernel_ms(1))
+                k_ms["match_prep"].append(ctx.spf_last_kernel_ms(2))
+            sync_all()
+        ctx.spf_check_fault()
+        return ev, k_ms, ctx.spf_launch_count() - launches0, clocks.summary(), bi
+
+    # a run that saw a hardware or thermal slowdown is rejected and measured once more (timing rules)
+    remeasured = False
+    ev, k_ms, launches, clk, best_idx = measure()
+    bad = sorted(set(clk["reasons"]) & {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"})
+    if bad:
+        remeasured = True
+        time.sleep(5.0)
+        ev, k_ms, launches, clk, best_idx = measure()
+        bad = sorted(set(clk["reasons"]) & {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"})
     if products is None:
         products = ctx.spf_last_match_products()
     total_ms = ev[0][0].elapsed_time(ev[-1][3])
@@ -279,8 +291,6 @@ def run_spf(args, cfg):
     prepare_ms, slice_ms, match_ms = part(0, 1), part(1, 2), part(2, 3)
     ms_per_step = total_ms / args.steps
     value = shard_units(cfg.n_img, world) / (ms_per_step * 1e-3)
-    clk = clocks.summary()
-    bad = sorted(set(clk["reasons"]) & {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"})
 
     # sanity statistic of the result (not a correctness check: tests/ do that)
     sel = planted >= 0
@@ -308,7 +318,8 @@ def run_spf(args, cfg):
             "slice_points_per_s": cfg.M * cfg.P * world / (slice_ms * 1e-3),
             "match_images_per_s": cfg.n_img * world / (match_ms * 1e-3),
             "roofline": kern[dominant]["roofline"], "kernels": kern, "peaks": peaks,
-            "clocks": {"sm_mhz": clk["sm_mhz"], "sm_max_mhz": clk["sm_max_mhz"], "reasons": clk["reasons"], "rejected_for": bad},
+            "clocks": {"sm_mhz": clk["sm_mhz"], "sm_max_mhz": clk["sm_max_mhz"], "reasons": clk["reasons"], "rejected_for": bad,
+                       "remeasured": remeasured},
             "gpu_launches": int(launches), "planted_hit_rate": hit}
 
     # end to end through the C-ABI host-buffer call (pinned host memory, copies inside the timed region)
