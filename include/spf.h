@@ -212,8 +212,8 @@ SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
 SPF_API int spf_check_fault(spf_ctx *ctx, void *stream);
 
 /*
- * Device-time statistics of the last spf_slice / spf_match, for bench.py: counts of launches
- * this library made since the context was created (so the harness can report gpu_launches).
+ * Number of launches of this library's OWN kernels since the context was created (cuFFT's kernels
+ * and memsets are not counted), so that the harness can report gpu_launches.
  */
 SPF_API int64_t spf_launch_count(const spf_ctx *ctx);
 

@@ -191,7 +191,7 @@ int spf_prepare_model(spf_ctx *ctx, const float *model, void *stream_) {
     cufftResult fr = cufftSetStream(ctx->plan, st);
     if (fr == CUFFT_SUCCESS) fr = cufftExecC2C(ctx->plan, (cufftComplex *)ctx->d_fft, (cufftComplex *)ctx->d_fft, CUFFT_FORWARD);
     if (fr != CUFFT_SUCCESS) return spf_set_err(ctx, SPF_ECUDA, "cufftExecC2C failed: %d", (int)fr);
-    ctx->launches++;
+    // (cuFFT's own kernels are not counted in spf_launch_count: it counts this library's kernels only)
     k_relayout<<<blocks, 256, 0, st>>>(ctx->d_fft, ctx->nf, ctx->np, ctx->sz, ctx->nf / 2 + ctx->halo, ctx->d_gridc, ctx->d_gridr);
     SPF_LAUNCH_CHECK(ctx);
     int bad = 1;
