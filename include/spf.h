@@ -186,7 +186,7 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *                  2 = the same tile, a warp per point: 32 lanes read an 8 x 8 window per x-plane with no
  *                      bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; w = 10 runs as 0);
  *                  3 = the warp-per-point gather straight from global memory (no TMA, mbarrier or tile;
- *                      w <= 8; w = 10 runs as 1)
+ *                      8 x 8 window at w = 7, 16-cell window at w = 10)
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
  *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused norm-add + argmin epilogue (the product);
  *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused

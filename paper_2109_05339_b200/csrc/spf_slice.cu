@@ -71,9 +71,10 @@ enum { IMPL_STAGED = 0, IMPL_GLOBAL = 1, IMPL_COOP = 2, IMPL_GCOOP = 3 };
 // flight per lane, then ONE multi-value butterfly (spf_slice_math.cuh: 4 + 2 + 1 exchanges halve the
 // value count while halving the lane group, 2 more finish) instead of eight 5-step reductions; lane
 // 4 u ends with point u's sum and the owner lanes fetch theirs.
-template <bool REAL, int BZ, typename IDX>
+template <bool REAL, int BZ, typename IDX, bool WIDE = false>
 __device__ __forceinline__ void coop_sweep(const float *tile, IDX cell, int S1, int bz, int w, const float *wts_warp, int lane,
                                            spfm::c2 &c) {
+    constexpr int STRIDE = WIDE ? SPF_COOPW_STRIDE : SPF_COOP_STRIDE;
     const int h = lane >> 3, k = lane & 7;
     for (int g0 = 0; g0 < 32; g0 += spfm::MR8) {
         float pr[spfm::MR8], pi[spfm::MR8];
@@ -81,8 +82,10 @@ __device__ __forceinline__ void coop_sweep(const float *tile, IDX cell, int S1, 
         for (int u = 0; u < spfm::MR8; ++u) {
             const IDX cell_p = __shfl_sync(0xffffffffu, cell, g0 + u);
             spfm::c2 part; part.x = part.y = 0.0f;
-            if (cell_p >= 0)    // warp-uniform: skips an empty slot of a ragged patch
-                part = spfm::gather_coop_lane<REAL, BZ, IDX>(tile, cell_p, S1, bz, w, wts_warp + (g0 + u) * SPF_COOP_STRIDE, h, k);
+            if (cell_p >= 0) {  // warp-uniform: skips an empty slot of a ragged patch
+                if (WIDE) part = spfm::gather_coop_lane_wide<REAL, IDX>(tile, cell_p, S1, bz, w, wts_warp + (g0 + u) * STRIDE, lane);
+                else part = spfm::gather_coop_lane<REAL, BZ, IDX>(tile, cell_p, S1, bz, w, wts_warp + (g0 + u) * STRIDE, h, k);
+            }
             pr[u] = part.x; pi[u] = part.y;
         }
 #pragma unroll
@@ -116,7 +119,10 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
     constexpr bool STAGED = (IMPL == IMPL_STAGED || IMPL == IMPL_COOP);
     constexpr bool COOP = (IMPL == IMPL_COOP);
     constexpr bool GCOOP = (IMPL == IMPL_GCOOP);
-    static_assert(!(COOP || GCOOP) || (W >= 2 && W <= 8), "the cooperative gather reads an 8 x 8 window per x-plane");
+    constexpr bool WIDE = GCOOP && W > 8;      // 16-cell window, global memory only (spf_slice_math.cuh)
+    static_assert(!COOP || (W >= 2 && W <= 8), "the staged cooperative gather reads an 8 x 8 window per x-plane");
+    static_assert(!GCOOP || (W >= 2 && W <= 12), "the cooperative gather handles 2 <= w <= 12");
+    constexpr int WSTRIDE = WIDE ? SPF_COOPW_STRIDE : SPF_COOP_STRIDE;
     constexpr int WMAX = W ? W : SPF_MAX_W;
     constexpr int E = REAL ? 1 : 2;            // floats per cell
     constexpr int CELL = 4 * E;                // bytes per cell
@@ -131,7 +137,7 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
     __shared__ uint32_t s_abort;
     extern __shared__ __align__(128) uint8_t s_dyn[];
     // cooperative variant: the first SPF_COOP_WTS_BYTES of dynamic shared memory hold the points' weights
-    uint8_t *s_tile = s_dyn + ((COOP || GCOOP) ? SPF_COOP_WTS_BYTES : 0);
+    uint8_t *s_tile = s_dyn + (COOP ? SPF_COOP_WTS_BYTES : 0);
 
     if (tid == 0) {
         spfm::quat_to_R(a.quats + 4 * m, sR);
@@ -195,14 +201,21 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
     spfm::c2 c;
     c.x = c.y = 0.0f;
     const int lane = tid & 31;
-    const float *wts_warp = reinterpret_cast<const float *>(s_dyn) + (tid & ~31) * SPF_COOP_STRIDE;
+    const float *wts_warp = reinterpret_cast<const float *>(s_dyn) + (tid & ~31) * WSTRIDE;
     if (COOP || GCOOP) {
         // every lane parks its point's weights where its warp will read them back
-        float pk[24];
-        spfm::coop_pack_weights<WMAX>(pk, w, wx, wy, wz);
-        float4 *dst4 = reinterpret_cast<float4 *>(reinterpret_cast<float *>(s_dyn) + tid * SPF_COOP_STRIDE);
+        float4 *dst4 = reinterpret_cast<float4 *>(reinterpret_cast<float *>(s_dyn) + tid * WSTRIDE);
+        if (WIDE) {
+            float pk[44];
+            spfm::coop_pack_weights_wide<WMAX>(pk, w, wx, wy, wz);
 #pragma unroll
-        for (int v = 0; v < 6; ++v) dst4[v] = make_float4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
+            for (int v = 0; v < 11; ++v) dst4[v] = make_float4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
+        } else {
+            float pk[24];
+            spfm::coop_pack_weights<WMAX>(pk, w, wx, wy, wz);
+#pragma unroll
+            for (int v = 0; v < 6; ++v) dst4[v] = make_float4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
+        }
         __syncwarp();
     }
     if (STAGED && staged) {
@@ -231,9 +244,10 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         // variant 2 whose box does not fit the tile.  The 8 x 8 window reads one row and one cell past the
         // w taps (weight 0): for finite input the last first-cell is np - 8 (spf_slice_math.cuh), so the
         // window ends at np - 1; the clamp only acts on the NaN / inf inputs cell_and_fraction parks at np - w.
-        const int qy = min(py, a.np - 8), qz = min(pz, a.np - 8);
+        // The wide form (w > 8) reads exactly the w x w taps: no clamp needed.
+        const int qy = WIDE ? py : min(py, a.np - 8), qz = WIDE ? pz : min(pz, a.np - 8);
         const long long cell = active ? ((long long)px * a.np + qy) * a.sz + qz : -1;
-        coop_sweep<REAL, 0, long long>(a.grid, cell, a.np * a.sz, a.sz, w, wts_warp, lane, c);
+        coop_sweep<REAL, 0, long long, WIDE>(a.grid, cell, a.np * a.sz, a.sz, w, wts_warp, lane, c);
         if (!active) return;
     } else {
         if (!active) return;
@@ -269,7 +283,7 @@ int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
     // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid (w = 7)
     uint32_t smem = 0;
     args.cap_bytes = 0;
-    if (IMPL == IMPL_GCOOP) smem = (uint32_t)SPF_COOP_WTS_BYTES;   // the parked weights only
+    if (IMPL == IMPL_GCOOP) smem = W > 8 ? (uint32_t)(SPF_PATCH * SPF_COOPW_STRIDE * 4) : (uint32_t)SPF_COOP_WTS_BYTES;   // the parked weights only
     if (IMPL == IMPL_STAGED || IMPL == IMPL_COOP) {
         // w = 10: an 8 x 16 patch needs up to 73 KB on the real grid (seeded replay of the Slicing-heavy geometry),
         // 72 KB stages all but a fraction of a percent of the blocks and still leaves three blocks per SM
@@ -300,6 +314,7 @@ int launch_slice_w(spf_ctx *ctx, SliceArgs &args, int impl, cudaStream_t st) {
             return launch_slice<7, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         case 10:   // 10 x 10 window: the cooperative form (8 x 8) does not apply
             if (impl == IMPL_STAGED || impl == IMPL_COOP) return launch_slice<10, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
+            if (impl == IMPL_GCOOP) return launch_slice<10, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
             return launch_slice<10, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         default: return launch_slice<0, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);  // any other width: runtime-w global gather
     }

@@ -240,6 +240,70 @@ SPF_HD c2 gather_coop_lane(const float *tile, IDX cell, int S1, int bz, int w, c
     return r;
 }
 
+// The warp-per-point gather for 8 < w <= 16 (variant 3 at w = 10, Slicing-heavy): the window is 16 cells wide
+// (lanes with k >= w stay idle and load nothing), so a warp covers 2 rows per load and needs ceil(w / 2) loads
+// per x-plane: rows h, h + 2, h + 4, ...  Weight layout per point (SPF_COOPW_STRIDE floats; 44 = 12 mod 32 keeps
+// the owners' 16-byte stores conflict-free):
+//   [0,16)  wz[0..15]            [16,32) wy[h + 2 i] at 16 + 8 h + i  (h = 0, 1; i = 0..7)            [32,48) wx[0..15]
+// only the first 44 are stored (wx[12..15] are never read: w <= 12 for this layout; w = 10 is what is built).
+#define SPF_COOPW_STRIDE 44
+template <int WMAX>
+SPF_HD void coop_pack_weights_wide(float (&out)[44], int w, const float (&wx)[WMAX], const float (&wy)[WMAX], const float (&wz)[WMAX]) {
+#pragma unroll
+    for (int v = 0; v < 44; ++v) out[v] = 0.0f;
+#pragma unroll
+    for (int t = 0; t < 12; ++t) {
+        if (t < WMAX) {
+            if (t < w) {
+                out[t] = wz[t < WMAX ? t : 0];
+                out[16 + 8 * (t & 1) + (t >> 1)] = wy[t < WMAX ? t : 0];
+                out[32 + t] = wx[t < WMAX ? t : 0];
+            }
+        }
+    }
+}
+
+// lane = (h, k), h = lane >> 4 in {0, 1}, k = lane & 15; NPASS = ceil(w / 2) <= 6 loads per x-plane
+template <bool REAL, typename IDX>
+SPF_HD c2 gather_coop_lane_wide(const float *grid, IDX cell, int S1, int rp, int w, const float *wts, int lane) {
+    constexpr int E = REAL ? 1 : 2;
+    constexpr int MAXPASS = 6;
+    c2 r; r.x = r.y = 0.0f;
+    const int h = lane >> 4, k = lane & 15;
+    if (k >= w) return r;
+    const int npass = (w + 1) >> 1;
+    const float *p0 = grid + (size_t)(cell + (IDX)(h * rp + k)) * E;
+    const size_t row2 = (size_t)(2 * rp) * E, plane = (size_t)S1 * E;
+    float ar[MAXPASS], ai[MAXPASS];
+#pragma unroll
+    for (int i = 0; i < MAXPASS; ++i) ar[i] = ai[i] = 0.0f;
+    for (int t1 = 0; t1 < w; ++t1) {
+        const float wxt = wts[32 + t1];
+#pragma unroll
+        for (int i = 0; i < MAXPASS; ++i) {
+            if (i < npass && h + 2 * i < w) {
+                if (REAL) ar[i] = fmaf(wxt, p0[i * row2], ar[i]);
+                else {
+                    const c2 v = *reinterpret_cast<const c2 *>(p0 + i * row2);
+                    ar[i] = fmaf(wxt, v.x, ar[i]); ai[i] = fmaf(wxt, v.y, ai[i]);
+                }
+            }
+        }
+        p0 += plane;
+    }
+    float sr = 0.0f, si = 0.0f;
+#pragma unroll
+    for (int i = 0; i < MAXPASS; ++i) {
+        if (i < npass) {
+            const float wyi = wts[16 + 8 * h + i];
+            sr = fmaf(wyi, ar[i], sr); si = fmaf(wyi, ai[i], si);
+        }
+    }
+    r.x = wts[k] * sr;
+    r.y = REAL ? 0.0f : wts[k] * si;
+    return r;
+}
+
 // Multi-value warp reduction used by the cooperative gather: every lane holds MR8 = 8 partial sums (one
 // per point of a group).  Exchange step with lane offset o = 16, 8, 4 and n = 4, 2, 1 values: a lane whose
 // bit o is set keeps values [n, 2n) and sends [0, n), the others the opposite, and adds what it receives;

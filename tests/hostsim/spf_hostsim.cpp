@@ -110,7 +110,7 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
         const bool any = hi[0] >= lo[0];
         const int Lx = any ? hi[0] - lo[0] + w : 0, Ly = any ? hi[1] - lo[1] + w : 0, Lz = any ? hi[2] - lo[2] + w : 0;
         spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, cap_bytes, coop != 0);
-        if (coop == 2) g.ok = false;        // variant 3: no tile at all
+        if (coop == 2 || (coop && w > 8)) g.ok = false;        // variant 3: no tile at all (and no staged cooperative form beyond w = 8)
         std::vector<float> tile;
         if (g.ok) {
             n_staged++;
@@ -129,16 +129,29 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
         spfm::c2 res[PATCH];
         if (coop) {
             // weights parked in the 28-float layout (slots of empty lanes hold NaN: they must never be read)
-            std::vector<float> wts((size_t)PATCH * SPF_COOP_STRIDE, std::nanf(""));
+            const bool wide = w > 8;                 // variant 3 at w = 10: 16-cell window, 44-float weight sets
+            const int wstride = wide ? SPF_COOPW_STRIDE : SPF_COOP_STRIDE;
+            std::vector<float> wts((size_t)PATCH * wstride, std::nanf(""));
             for (int t = 0; t < PATCH; ++t) {
-                float pk[24];
-                spfm::coop_pack_weights<SPF_MAX_W>(pk, w, wx[t], wy[t], wz[t]);
-                for (int v = 0; v < 24; ++v) wts[(size_t)t * SPF_COOP_STRIDE + v] = jj[t] >= 0 ? pk[v] : std::nanf("");
+                if (wide) {
+                    float pk[44];
+                    spfm::coop_pack_weights_wide<SPF_MAX_W>(pk, w, wx[t], wy[t], wz[t]);
+                    for (int v = 0; v < 44; ++v) wts[(size_t)t * wstride + v] = jj[t] >= 0 ? pk[v] : std::nanf("");
+                } else {
+                    float pk[24];
+                    spfm::coop_pack_weights<SPF_MAX_W>(pk, w, wx[t], wy[t], wz[t]);
+                    for (int v = 0; v < 24; ++v) wts[(size_t)t * wstride + v] = jj[t] >= 0 ? pk[v] : std::nanf("");
+                }
             }
             // one lane's partial sum for point t: from the staged tile, or (variant 3, and blocks of variant 2
             // whose box does not fit) straight from the padded grid with the y / z clamp of the kernel
             auto lane_part = [&](int t, int lane) {
-                const float *wt = &wts[(size_t)t * SPF_COOP_STRIDE];
+                const float *wt = &wts[(size_t)t * wstride];
+                if (wide) {      // exactly the w x w taps: no clamp
+                    const long long cell = ((long long)px[t] * np + py[t]) * sz + pz[t];
+                    return is_real ? spfm::gather_coop_lane_wide<true, long long>(grid, cell, np * sz, sz, w, wt, lane)
+                                   : spfm::gather_coop_lane_wide<false, long long>(grid, cell, np * sz, sz, w, wt, lane);
+                }
                 if (g.ok) {
                     const int cell = (px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2]);
                     return is_real ? spfm::gather_coop_lane<true, 0, int>(tile.data(), cell, g.S1, g.bz, w, wt, lane >> 3, lane & 7)

@@ -333,6 +333,26 @@ def test_staged_block_replay_wide_kernel(sim):
         assert _rel(c.real if is_real else c, ref.real if is_real else ref) <= SLICE_TOL
 
 
+def test_wide_warp_per_point_replay(sim):
+    """w = 10 through variant 3's 16-cell window (2 rows x 16 cells per load, idle lanes beyond the 10th cell, 44-float
+    weight sets): real and complex grid against the oracle, and against the one-thread-per-point sum."""
+    rng = np.random.default_rng(9)
+    N = 21
+    w, nf, halo = _plan(N, 1e-9)
+    pix = make_detector(1, 32)[:1000]               # ragged: the last patch is partly empty
+    refs = random_quaternions(4, seed=31)
+    table = _patch_table(sim, 0, 0, 0, 1000)
+    for is_real in (1, 0):
+        A = make_model(N, 12, 5.0) if is_real else rng.standard_normal((N, N, N)).astype(np.float32)
+        g, npad, sz = _padded_grid(sim, A, w, nf, halo)
+        c, stats = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, 2)
+        assert np.isfinite(c.view(np.float32)).all() and stats[0] == 0
+        ref = orc.slice_points(A, refs, pix)
+        assert _rel(c.real if is_real else c, ref.real if is_real else ref) <= SLICE_TOL
+        direct = _slice(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, 1)
+        assert _rel(c, direct) <= 2e-6
+
+
 def test_staged_block_replay_paper_scale_sampled(sim):
     """Paper-scale model and detector (8 x 16 lattice patches of 4 x 128 x 128 pixels), 4 orientations through the
     warp-per-point path: every block must fit the 48 KB tile (no fallback), 2,048 sampled pairs from the oracle."""
