@@ -126,7 +126,7 @@ SPF_HD c2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMA
     constexpr int E = REAL ? 1 : 2;
     // the outer tap loop is unrolled for the compile-time widths up to 8 (wx[] then stays in registers);
     // for wider or run-time widths it stays a loop and wx[] is indexed in local memory
-#pragma unroll
+#pragma unroll(WMAX <= 8 ? WMAX : 1)
     for (int t1 = 0; t1 < (WMAX <= 8 ? WMAX : w); ++t1) {
         if (WMAX <= 8 && t1 >= w) break;
         float pr = 0.0f, pi = 0.0f;
