@@ -1,6 +1,6 @@
 """bench.py -- one JSON line for the M-TIP orientation-matching hot path on B200 (contract: DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config paper_scale] [--impl spf|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config paper_scale] [--impl spf|reference] [--native]
 
 A "step" is one pass of the whole hot path over one batch of
 synthetic input: spf_prepare_model -> spf_slice (M x P points) -> spf_match (n_img x M x P).
@@ -8,7 +8,7 @@ synthetic input: spf_prepare_model -> spf_slice (M x P points) -> spf_match (n_i
   e2e     the same through spf_orientation_match_host with pinned HOST buffers (copies inside the timed region)
   roofline / kernels   per-kernel device times (CUDA events recorded by the library on the launching stream)
   cpu_baseline   the oracle, as it stands, timed on this box's host cores on a bounded sample (rank 0, N = 1)
-N > 1 (torchrun): images are partitioned across ranks, the model and all M orientations replicated --
+N > 1 (under torchrun, or plain `python bench.py --gpus N`, which re-launches itself under torchrun): images are partitioned across ranks, the model and all M orientations replicated --
 the paper's scheme; no data-path collective; "scaling": "weak".
 --impl reference times the oracle (oracle/) on a bounded sample of the same workload.
 """
@@ -31,8 +31,8 @@ from spf_inputs import (CONFIGS, make_model, make_detector, make_mask, random_qu
 
 METRIC = "orientation-matched images/sec (whole step: prepare + slice + match)"
 UNIT = "images/s"
-ORACLE_POINTS = 16384     # NUDFT sample of the cpu_baseline / reference arm (about 10 s on 8 cores at N = 151)
-ORACLE_IMAGES = 32        # images x all M slices brute-forced by the oracle (about 10 s on 8 cores at M = 10,000)
+ORACLE_POINTS = 8192      # NUDFT sample of the cpu_baseline / reference arm (>= 4,096; about 6 s on 8 cores at N = 151)
+ORACLE_IMAGES = 64        # images x ALL M slices brute-forced by the oracle (>= 64; about 15 s on 8 cores at M = 10,000)
 
 
 def _peaks():
@@ -140,18 +140,29 @@ def dist_max(x, dist=None):
 # ------------------------------------------------------------------------------------------------
 # the oracle on a bounded sample (cpu_baseline leg and --impl reference; the only places oracle/ runs)
 # ------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, model, pix, mask, refs, n_points, n_images, m_slices):
+def oracle_match_inputs(cfg, pix, n_images, m_slices):
+    """Inputs of the oracle's matching sample (the oracle cannot slice M x P points here): surrogate model images
+    generated 1,000 rows at a time (each block its own seed, so the fp64 temporaries stay small) and Poisson images
+    drawn from evenly spaced rows."""
+    from spf_inputs import surrogate_slices
+    S = np.empty((m_slices, cfg.P), np.float32)
+    for s0 in range(0, m_slices, 1000):
+        n = min(1000, m_slices - s0)
+        S[s0:s0 + n] = surrogate_slices(n, pix, seed=5 + s0)
+    S *= np.float32(cfg.photons / max(float(S[:min(m_slices, 1000)].sum(axis=1, dtype=np.float64).mean()), 1e-30))
+    I = poisson_images(S[(np.arange(n_images) * max(1, m_slices // max(1, n_images))) % m_slices])
+    return I, S
+
+
+def oracle_sample(cfg, model, pix, mask, refs, n_points, n_images, m_slices, match_inputs=None):
     """Times oracle NUDFT on n_points sampled (orientation, pixel) pairs and oracle brute-force matching of
     n_images images against m_slices model images of P pixels; extrapolates to the whole step."""
     from oracle import oracle as orc
-    from spf_inputs import surrogate_slices
     sm, sj = sample_pairs(cfg.M, cfg.P, n_points)
     t0 = time.perf_counter()
     orc.slice_points(model, refs, pix, sm, sj)
     t_slice = time.perf_counter() - t0
-    S = surrogate_slices(m_slices, pix)             # inputs for the matching sample (the oracle cannot slice M x P here)
-    S *= np.float32(cfg.photons / max(float(S.sum(axis=1).mean()), 1e-30))
-    I = poisson_images(S[np.arange(n_images) % m_slices])
+    I, S = match_inputs if match_inputs is not None else oracle_match_inputs(cfg, pix, n_images, m_slices)
     t0 = time.perf_counter()
     orc.match(I, S, mask)
     t_match = time.perf_counter() - t0
@@ -172,10 +183,11 @@ def run_reference(args, cfg):
     model, pix, mask, refs, _, _ = host_inputs(cfg)
     scale = min(1.0, 8.0 / max(1, args.steps + args.warmup))     # keep the whole run within a few minutes
     n_pts, n_im = max(1024, int(ORACLE_POINTS * scale)), max(4, int(ORACLE_IMAGES * scale))
-    m_s = min(cfg.M, 2000)
+    m_s = cfg.M if cfg.M <= 20_000 else 20_000                   # all M slices (host memory bounds the largest config)
+    inputs = oracle_match_inputs(cfg, pix, n_im, m_s)            # generated once, outside every timed sample
     last, times = None, []
     for it in range(args.warmup + args.steps):
-        last = oracle_sample(cfg, model, pix, mask, refs, n_pts, n_im, m_s)
+        last = oracle_sample(cfg, model, pix, mask, refs, n_pts, n_im, m_s, inputs)
         if it >= args.warmup:
             times.append(last)
     value = float(np.mean([t["value"] for t in times]))
@@ -215,10 +227,12 @@ def run_spf(args, cfg):
     model, pix, mask, refs, truth, planted = host_inputs(cfg, rank)
     ctx = SpfContext(cfg.N, eps=cfg.eps, device=local)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    # kernel variants: the faster ones (TMA-staged gather -- the fastest verified form --, cta_group::2 GEMM) where their device self-check
-    # passes in a child process, else the library defaults (paper_2109_05339_b200/selfcheck.py)
-    variants = ({"slice_staged": False, "slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False, "slice_impl": 1,
-                 "match_impl": 1, "match_cta_group": 1} if args.no_autotune else ctx.spf_autotune())
+    # kernel variants: the library defaults, or with --native the faster ones (TMA-staged gather, tcgen05 GEMM) whose
+    # device self-check passes in a child process (paper_2109_05339_b200/selfcheck.py).  Opt-in until those kernels
+    # have been cleared on hardware: the default run never launches an unverified kernel.
+    variants = (ctx.spf_autotune() if args.native else
+                {"slice_staged": False, "slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False,
+                 "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
     info = ctx.info
     d_model = torch.from_numpy(model).to(dev)
     d_pix, d_refs = torch.from_numpy(pix).to(dev), torch.from_numpy(refs).to(dev)
@@ -255,7 +269,6 @@ def run_spf(args, cfg):
     def measure():
         """EXACTLY args.steps timed steps between two barriers; CUDA events on the current stream; clocks sampled."""
         ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-        k_ms = {"slice": [], "gemm": [], "match_prep": []}
         sync_all()
         launches0 = ctx.spf_launch_count()
         with ClockSampler(physical_gpu_index(local)) as clocks:
@@ -267,12 +280,23 @@ def run_spf(args, cfg):
                 ev[k][2].record()
                 bi, bd = ctx.spf_match(images, slices, d_mask)
                 ev[k][3].record()
-                k_ms["slice"].append(ctx.spf_last_kernel_ms(0))       # these synchronise on the library's own events
+            sync_all()
+            launches = ctx.spf_launch_count() - launches0
+            # Per-kernel device times: the library's own CUDA events around the dominant kernels (recorded on the
+            # launching stream).  Reading them synchronises the host, so they are taken in a SECOND pass of the same
+            # steps, after the timed region has closed and still under the clock sampler -- `value` has no host
+            # bubbles, and each kernel's time is the mean over args.steps launches.
+            k_ms = {"slice": [], "gemm": [], "match_prep": []}
+            for k in range(args.steps):
+                ctx.spf_prepare_model(d_model)
+                ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=alpha, out=slices)
+                ctx.spf_match(images, slices, d_mask)
+                k_ms["slice"].append(ctx.spf_last_kernel_ms(0))
                 k_ms["gemm"].append(ctx.spf_last_kernel_ms(1))
                 k_ms["match_prep"].append(ctx.spf_last_kernel_ms(2))
-            sync_all()
+            torch.cuda.synchronize()
         ctx.spf_check_fault()
-        return ev, k_ms, ctx.spf_launch_count() - launches0, clocks.summary(), bi
+        return ev, k_ms, launches, clocks.summary(), bi
 
     # a run that saw a hardware or thermal slowdown is rejected and measured once more (timing rules)
     remeasured = False
@@ -309,7 +333,7 @@ def run_spf(args, cfg):
                        "kernel_variants": {"slice": {0: "tma_staged, thread per point", 1: "global_gather, thread per point",
                                                      2: "tma_staged, warp per point", 3: "global_gather, warp per point"}[variants["slice_impl"]],
                                            "match": ("tcgen05 cta_group::%d" % variants["match_cta_group"]) if variants["match_impl"] == 0
-                                                    else "cuda_core difference form (tcgen05 self-check did not pass)",
+                                                    else "cuda_core difference form (library default; tcgen05 variant %s)" % ("failed its self-check" if args.native else "not requested"),
                                            "selfcheck": variants},
                        "parallelism": "images partitioned x%d, orientations replicated" % world,
                        "l2": "inputs larger than L2 (slices %.2f GB, images %.2f GB per step; no flush needed)"
@@ -332,7 +356,7 @@ def run_spf(args, cfg):
             line["e2e"] = {"value": None, "unit": UNIT, "error": repr(e)[:200]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         try:
-            base = oracle_sample(cfg, model, pix, mask, refs, ORACLE_POINTS, ORACLE_IMAGES, min(cfg.M, 2000))
+            base = oracle_sample(cfg, model, pix, mask, refs, ORACLE_POINTS, ORACLE_IMAGES, cfg.M if cfg.M <= 20_000 else 20_000)
             line["cpu_baseline"] = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample", "slice_points_per_s", "match_pairs_per_s")}
         except Exception as e:
             line["cpu_baseline"] = {"value": None, "unit": UNIT, "kind": "oracle", "error": repr(e)[:200]}
@@ -389,14 +413,21 @@ def roofline_objects(cfg, info, k_ms, products, peaks, clk):
                                     "unit": "TFLOP/s", "frac": ach / peaks["tensor_tflops"], "traffic": None,
                                     "peak_source": "%s sustained bf16 cuBLAS (fp16 = bf16 rate)" % peaks["source"]}}
     else:
-        # CUDA-core matcher (the tcgen05 kernel did not pass its self-check): one subtract + one FMA per pixel pair
+        # CUDA-core matcher (library default): one FADD (the difference) + one FFMA (square and add) per pixel pair =
+        # 3 flop in 2 issue slots.  Peak = the fp32 FMA pipe (guide: 128 lanes/clk/SM, 2 flop per FFMA); this
+        # instruction mix can reach at most 3/4 of it, which `mix_ceiling` states -- no credit is taken for it.
         ach = 3.0 * cfg.n_img * cfg.M * cfg.P / t_g / 1e12
         out["gemm"] = {"ms": t_g * 1e3, "products": 0, "algorithmic_tflops_fp32_equivalent": alg / t_g / 1e12,
                        "images_per_s": cfg.n_img / t_g,
-                       "roofline": {"kernel": "k_match_simt", "bound": "alu", "achieved": ach, "peak": alu_peak * 0.75,
-                                    "unit": "TFLOP/s", "frac": ach / (alu_peak * 0.75), "traffic": None,
-                                    "peak_source": "148 SM x 128 lanes x sm_max_mhz x 1.5 flop per instruction slot "
-                                                   "(FADD = 1 flop, FFMA = 2 flop alternate)"}}
+                       "roofline": {"kernel": "k_match_simt", "bound": "alu", "achieved": ach, "peak": alu_peak,
+                                    "unit": "TFLOP/s", "frac": ach / alu_peak, "traffic": None, "mix_ceiling": 0.75,
+                                    "peak_source": "fp32 FMA pipe: %d SM x 128 lanes x 2 flop x sm_max_mhz (DESIGN.md section 6); "
+                                                   "FADD + FFMA per pixel pair = 3 flop per 2 slots, so <= 0.75 of it"
+                                                   % info.sm_count}}
+    if not products:
+        # the CUDA-core matcher has no operand preparation (only a memset of the argmin keys): nothing to report
+        out["match_prep"] = {"ms": None, "roofline": None, "skipped": "no operand preparation ran (CUDA-core matcher)"}
+        return out
     t_p = float(np.mean(k_ms["match_prep"])) * 1e-3
     prep_bytes = (cfg.n_img + cfg.M) * cfg.P * 4.0 * 2 + (cfg.n_img + cfg.M) * Ppad * 4.0   # abs-max read + split read + 2 fp16 planes written
     out["match_prep"] = {"ms": t_p * 1e3,
@@ -434,21 +465,66 @@ def run_e2e(args, cfg, ctx, model, refs, pix, mask, images_dev, alpha, world, di
             "timer": "host clock around the synchronous C-ABI call spf_orientation_match_host (max over ranks)"}
 
 
+def respawn_under_torchrun(args, argv):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: re-exec the same command line as
+    `python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py ...`
+    (one rank per GPU), so the plain command the driver uses for N = 1 also works for N > 1.  Returns the exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")          # keep NCCL's communicator log on: the rank check reads it
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    sys.stderr.write("bench.py: --gpus %d without WORLD_SIZE: re-launching under torchrun (port %d)\n" % (args.gpus, port))
+    return subprocess.call(cmd, env=env)
+
+
+def run_hostcheck(args):
+    """--impl hostcheck (CPU test of the N > 1 launch path, tests/test_bench_host.py): rendezvous over gloo, shard the
+    units, take the max-over-ranks of a per-rank number, rank 0 prints one line.  No CUDA call, no kernel, no oracle."""
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    cfg = CONFIGS[args.config]
+    t = dist_max(10.0 + 5.0 * rank, dist if world > 1 else None)
+    if rank == 0:
+        print(json.dumps({"impl": "hostcheck", "n_gpus": world, "ranks_seen_max_ms": t, "units": shard_units(cfg.n_img, world),
+                          "scaling": "weak"}), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="spf", choices=["spf", "reference"])
+    ap.add_argument("--impl", default="spf", choices=["spf", "reference", "hostcheck"])
     ap.add_argument("--config", default="paper_scale", choices=sorted(CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiler runs)")
-    ap.add_argument("--no-autotune", action="store_true", help="library default kernel variants, no device self-check")
+    ap.add_argument("--native", action="store_true",
+                    help="self-check the TMA / tcgen05 kernel variants in child processes and use the ones that pass "
+                         "(opt-in until cleared on hardware; default: the library's default kernels only)")
+    ap.add_argument("--no-autotune", action="store_true", help="(default behaviour now; kept for old command lines)")
     args = ap.parse_args()
     if args.steps < 1:
         raise SystemExit("--steps must be >= 1")
     cfg = CONFIGS[args.config]
-    if args.impl == "reference":
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        raise SystemExit(respawn_under_torchrun(args, sys.argv[1:]))
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus and args.impl != "reference":
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%s" % (args.gpus, os.environ["WORLD_SIZE"]))
+    if args.impl == "hostcheck":
+        run_hostcheck(args)
+    elif args.impl == "reference":
         run_reference(args, cfg)
     else:
         if args.warmup < 3:

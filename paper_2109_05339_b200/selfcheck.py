@@ -14,8 +14,17 @@ matcher (`spf_match_reference`) -- on seeded random inputs that span several til
 tail.  This is a consistency check between two CUDA paths, not parity: parity against the oracle
 is what tests/ does.  Nothing here touches `oracle/`.
 
-Exit status of the child: 0 = variant agrees, 1 = disagrees or raised, anything else (signal,
-time-out) = faulted.
+Exit status of the child: 0 = variant agrees, 1 = disagrees with the reference kernels or the library's
+watchdog reported SPF_EFAULT (a verdict about the kernel), 3 = the check itself could not run (import error,
+out of memory, any other exception: no verdict), anything else (signal, time-out) = the process died or hung.
+
+Containment: `verified_variants` stops at the FIRST child that died or hung -- a kernel that raises an SM
+exception must not be followed by four more launches of unverified kernels on the same device -- and marks
+every remaining variant unverified.  Only verdicts (status 0 and 1) are cached on disk; a time-out or an
+infrastructure error is retried by the next process.
+
+The whole mechanism is OPT-IN (SpfContext.spf_autotune, bench.py --native, SPF_NATIVE=1 for tests/ and
+smoke()): until a variant has passed on hardware the library's defaults are the only kernels launched.
 """
 import json
 import os
@@ -23,7 +32,8 @@ import subprocess
 import sys
 import time
 
-VARIANTS = ("match_cg1", "slice_gcoop", "slice_staged", "slice_coop", "match_cg2")
+# least machinery first: classic CUDA (no TMA / mbarrier / tcgen05), then TMA + mbarrier, then tcgen05, CTA pairs last
+VARIANTS = ("slice_gcoop", "slice_staged", "slice_coop", "match_cg1", "match_cg2")
 SLICE_IMPL = {"slice_staged": 0, "slice_coop": 2, "slice_gcoop": 3}
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
@@ -186,8 +196,9 @@ def check_in_child(variant: str, device: int = 0, timeout_s: float = 240.0) -> d
             except ValueError:
                 pass
     tail = [ln for ln in lines if not ln.startswith("[selfcheck-json] ")][-3:]
-    return {"ok": status == 0, "status": status, "detail": " | ".join(tail)[-400:], "seconds": round(time.time() - t0, 1),
-            "metrics": metrics}
+    kind = "agrees" if status == 0 else ("disagrees" if status == 1 else ("no_verdict" if status == 3 else "died"))
+    return {"ok": status == 0, "status": status, "kind": kind, "detail": " | ".join(tail)[-400:],
+            "seconds": round(time.time() - t0, 1), "metrics": metrics}
 
 
 def fastest_slice_impl(report: dict) -> int:
@@ -240,25 +251,45 @@ def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = 
         except Exception:
             disk = {}
     out = {}
+    stopped_by = None
     for v in VARIANTS:
         key = (v, device)
         if key not in _cache:
-            if v in disk and isinstance(disk[v], dict) and "ok" in disk[v]:
+            if stopped_by is not None:
+                # not cached (in the process or on disk): a later process starts again from the variant that died
+                r = {"ok": False, "status": None, "kind": "not_run", "seconds": 0.0, "metrics": {},
+                     "detail": "not launched: the check of %s died or hung before it" % stopped_by}
+                sys.stderr.write("[libspf selfcheck] %-12s NOT RUN (%s)\n" % (v, r["detail"]))
+                out[v] = False
+                if report is not None:
+                    report[v] = r
+                continue
+            if v in disk and isinstance(disk[v], dict) and disk[v].get("kind") in ("agrees", "disagrees"):
                 _cache[key] = disk[v]
                 sys.stderr.write("[libspf selfcheck] %-12s %s (cached verdict from %s)\n" % (v, "ok" if disk[v]["ok"] else "FAILED", path))
             else:
-                _cache[key] = check_in_child(v, device, timeout_s)
+                r = check_in_child(v, device, timeout_s)
                 sys.stderr.write("[libspf selfcheck] %-12s %s (%s, %.1f s)\n" % (
-                    v, "ok" if _cache[key]["ok"] else "FAILED status %s" % _cache[key]["status"], _cache[key]["detail"],
-                    _cache[key]["seconds"]))
-                disk[v] = _cache[key]
-                if path:
-                    try:
-                        with open(path + ".tmp", "w") as f:
-                            json.dump(disk, f)
-                        os.replace(path + ".tmp", path)
-                    except Exception:
-                        pass
+                    v, "ok" if r["ok"] else "FAILED status %s (%s)" % (r["status"], r["kind"]), r["detail"], r["seconds"]))
+                if r["kind"] == "died":
+                    stopped_by = v
+                if r["kind"] in ("agrees", "disagrees", "died"):
+                    _cache[key] = r          # a kernel that died is not launched again by THIS process ...
+                if r["kind"] in ("agrees", "disagrees"):
+                    disk[v] = r              # ... but only verdicts persist across processes
+                    if path:
+                        try:
+                            with open(path + ".tmp", "w") as f:
+                                json.dump(disk, f)
+                            os.replace(path + ".tmp", path)
+                        except Exception:
+                            pass
+                out[v] = r["ok"]
+                if report is not None:
+                    report[v] = r
+                continue
+        elif _cache[key].get("kind") == "died":
+            stopped_by = stopped_by or v
         out[v] = _cache[key]["ok"]
         if report is not None:
             report[v] = _cache[key]
@@ -280,6 +311,11 @@ if __name__ == "__main__":
         text, metrics = run_variant(a.variant, a.device)
         print("[selfcheck-json] " + json.dumps(metrics))
         print("[selfcheck] %s: %s" % (a.variant, text))
-    except Exception as e:   # disagreement, SPF_EFAULT from the watchdog, CUDA error
+    except AssertionError as e:   # the variant disagrees with the reference kernels: a verdict
         print("[selfcheck] %s FAILED: %s: %s" % (a.variant, type(e).__name__, e))
         sys.exit(1)
+    except Exception as e:
+        # SPF_EFAULT (the kernel's watchdog gave up) is a verdict about the kernel; anything else (import error,
+        # out of memory, a CUDA error from an unrelated call) is not
+        print("[selfcheck] %s FAILED: %s: %s" % (a.variant, type(e).__name__, e))
+        sys.exit(1 if getattr(e, "status", None) == -5 else 3)

@@ -42,6 +42,27 @@ def test_two_ranks_shard_images_and_take_the_max_time():
     assert r0[3] != r1[3]                          # images (truth orientations) differ per rank
 
 
+def test_plain_gpus_2_relaunches_itself_under_torchrun():
+    """`python bench.py --gpus 2` with no torchrun environment must run 2 ranks through the same entry the driver
+    uses.  --impl hostcheck keeps it on the CPU: gloo rendezvous, max over ranks, one line."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "hostcheck", "--config", "tiny"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [l for l in p.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                       # rank 0 only
+    j = json.loads(lines[0])
+    assert j["n_gpus"] == 2 and j["ranks_seen_max_ms"] == 15.0 and j["units"] == 2 * 16
+    assert "re-launching under torchrun" in p.stderr
+
+
+def test_gpus_must_match_world_size():
+    env = dict(os.environ, RANK="0", WORLD_SIZE="2")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--impl", "hostcheck"],
+                       capture_output=True, text=True, timeout=120, cwd=ROOT, env=env)
+    assert p.returncode != 0 and "WORLD_SIZE" in p.stderr
+
+
 def test_dist_max_without_a_process_group_is_the_identity():
     assert bench.dist_max(3.5, None) == 3.5
 
@@ -76,6 +97,12 @@ def test_roofline_arithmetic_matches_design_md():
     assert abs(k2["slice"]["roofline"]["achieved"] - 2 * s["achieved"]) < 1e-3
     assert abs(k2["slice"]["alu"]["achieved"] - 2 * alu["achieved"]) < 1e-6
     assert abs(k2["gemm"]["roofline"]["achieved"] - 1.5 * g["achieved"]) < 1e-6
+    # CUDA-core matcher (products == 0): ALU roofline against the plain fp32 FMA peak, no operand-preparation entry
+    k3 = bench.roofline_objects(cfg, info, k_ms, 0, peaks, {"sm_mhz": None})
+    r3 = k3["gemm"]["roofline"]
+    assert r3["bound"] == "alu" and abs(r3["peak"] - alu["peak"]) < 1e-9 and r3["mix_ceiling"] == 0.75
+    assert abs(r3["achieved"] - 3.0 * 1e4 * 1e4 * 65_536 / 38.5e-3 / 1e12) < 1e-6
+    assert k3["match_prep"]["roofline"] is None and k3["match_prep"]["ms"] is None
 
 
 def test_reference_arm_prints_one_contract_line():

@@ -6,7 +6,15 @@ thread / one warp per point) and
 distances <= 1e-4, argmin exact outside near-ties.  Before a variant is launched in this process its
 device self-check (paper_2109_05339_b200/selfcheck.py) must have passed in a child process; if it did
 not, the test fails there, with the child's report, without launching the variant here.
+
+OPT-IN: these kernels have not yet passed on hardware, and an earlier GPU session of
+this repository raised SM exceptions that were never traced to a kernel.  Until the first-contact protocol
+(profiles/r02_first_contact.md) has cleared a variant, this file runs only with SPF_NATIVE=1 in the
+environment; otherwise every test here is SKIPPED, loudly, and the default `pytest -m gpu` launches the
+library's default kernels only.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -22,6 +30,8 @@ pytestmark = [pytest.mark.gpu, pytest.mark.timeout(1500)]
 
 @pytest.fixture(scope="module")
 def verified(spf):
+    if os.environ.get("SPF_NATIVE", "0") != "1":
+        pytest.skip("TMA / tcgen05 kernel variants are opt-in until cleared on hardware: set SPF_NATIVE=1 (DESIGN.md section 0)")
     from paper_2109_05339_b200 import selfcheck
     report = {}
     selfcheck.verified_variants(0, report=report)

@@ -1,7 +1,7 @@
 """GPU parity at the two largest configurations (-m gpu; collected last): BASELINE.json:configs[3] Matching-heavy
 and configs[4] Slicing-heavy at their FULL sizes, on sampled outputs the oracle can compute one by one.
 
-They run with whatever `spf_autotune` verified on the device (as bench.py does) and stress what the smaller
+They run with the library defaults, or with whatever `spf_autotune` verified on the device when SPF_NATIVE=1 (as bench.py --native does), and stress what the smaller
 configurations cannot: 64-bit indexing (6.55e9 slice values, 26 GB), 100,000-orientation argmin merges across
 391 slice tiles, the w = 10 kernel (eps = 1e-9; the parity bar stays 1e-5, reading s11) on a 405^3 fine grid.
 """
@@ -13,7 +13,7 @@ from oracle import oracle as orc
 from spf_inputs import (CONFIGS, make_model, make_detector, make_mask, random_quaternions, photon_scale, poisson_images,
                         surrogate_slices, sample_pairs)
 
-from test_gpu_parity import spf, _dev, _rel_l2, SLICE_TOL, DIST_TOL  # noqa: F401  (fixture)
+from test_gpu_parity import spf, _dev, _rel_l2, SLICE_TOL, DIST_TOL, choose_variants  # noqa: F401  (fixture)
 
 pytestmark = [pytest.mark.gpu, pytest.mark.timeout(2400)]
 
@@ -35,7 +35,7 @@ def test_slicing_heavy_sampled(spf):
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
     assert ctx.info.w == 10
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    print("slicing-heavy runs with", ctx.spf_autotune())
+    print("slicing-heavy runs with", choose_variants(ctx))
     ctx.spf_prepare_model(_dev(model))
     assert ctx.info.grid_is_real == 1
     sm, sj = sample_pairs(cfg.M, cfg.P, 2048)
@@ -64,7 +64,7 @@ def test_matching_heavy_sampled(spf):
     pix = make_detector(cfg.panels, cfg.panel_edge)
     mask = make_mask(cfg.panels, cfg.panel_edge, cfg.masked_frac)
     ctx = spf.SpfContext(8)
-    print("matching-heavy runs with", ctx.spf_autotune())
+    print("matching-heavy runs with", choose_variants(ctx))
     S = torch.empty((cfg.M, cfg.P), dtype=torch.float32, device="cuda")
     step = 10_000
     for s in range(0, cfg.M, step):                       # surrogate slices in blocks, each block its own seed
