@@ -135,11 +135,15 @@ SPF_API int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const float *
  * workspace [dev]: at least spf_match_workspace_bytes(n_img, M, P) bytes, 1024-byte aligned.
  *   d_{i,m} = sum_{j: mask_j} (I_ij - S_mj)^2,  best_idx[i] = argmin_m d_{i,m} (lowest m on
  *   exact ties of the computed fp32 distances), best_dist[i] = that distance.
- * With option match_impl = 0: evaluated as ||I||^2 + ||S||^2 - 2 I.S with the cross term on the
- * tensor cores from two-term fp16 splits of both operands (fp32-equivalent products, fp32
- * accumulation); values must satisfy |x| < 2^100 (they are rescaled by powers of two into fp16
- * range); where d is a tiny fraction of ||I||^2 + ||S||^2 the expansion cancels in fp32 and the
- * error is bounded by 1e-6 (||I||^2 + ||S||^2) instead of 1e-4 d (reading s14).
+ * With option match_impl = 0 (the tcgen05 matcher): evaluated as the conditioned expansion
+ *   d = ||I - c||^2 + sum S'(S' + 2c) - 2 I.S',  S' = S - c,  c = the mean of up to 1,024 evenly spaced slices
+ * (identical to the definition in exact arithmetic for any c), the cross term I.S' on the tensor
+ * cores from two-term fp16 splits of both operands (fp32-equivalent products, fp32 accumulation), the three terms
+ * added in fp64.  That decides the argmin; best_dist is then recomputed for the winner as the sum of squared
+ * differences (fp64 sum, rounded once), so it is within fp32 round-off of the definition in every case.  Values must
+ * satisfy |x| < 2^100 (they are rescaled by powers of two into fp16 range).  Two slices whose true distances to an
+ * image differ by less than about 1e-6 (||I - c||^2 + ||S'||^2) can be ranked either way by the tensor-core pass
+ * (reading s16); on the Poisson configurations that is far below the 1e-4 d near-tie window.
  * With match_impl = 1 (the library's starting value): the sum of squared differences as
  * written, in fp32 on the CUDA cores.  Either way the distance matrix is never written to
  * memory.  Requires M >= 1 when n_img >= 1.
@@ -192,9 +196,15 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused
  *                      argmin -- about 20x slower at Paper-scale, no tensor-core, TMA or mbarrier machinery
  *   "match_cta_group": CTAs per tcgen05 MMA (match_impl 0): 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
- * The defaults are the variants with the least machinery; the faster ones (slice_impl 0 / 2 / 3, match_impl 0,
- * match_cta_group 2) are switched on by the caller once they have been checked on the device at hand (the Python binding's
- * SpfContext.spf_autotune does that in a child process).
+ *   "match_chunk_kblocks": [32] 64-pixel K blocks accumulated inside TMEM before the epilogue warps add the chunk to
+ *                  their fp32 registers with round-to-nearest adds; 0 = all of K in TMEM (spf_match_math.cuh)
+ *   "match_condition": [1] = subtract the common vector c from the slices before the contraction; 0 = c = 0 (the plain
+ *                  expansion ||I||^2 + ||S||^2 - 2 I.S)
+ *   "match_refine": [1] = recompute the winner's distance in the difference form; 0 = return the epilogue's own value
+ * The defaults are the variants with the least machinery (classic CUDA: no TMA, mbarrier or tcgen05).  The others
+ * have not yet run on hardware and are opt-in: the caller switches them on once they have been
+ * checked on the device at hand (the Python binding's SpfContext.spf_autotune does that in a child process,
+ * DESIGN.md section 7).
  *   "record_events": [0]; 1 = spf_slice / spf_match record CUDA events on their stream around the
  *                    dominant kernels, read back with spf_last_kernel_ms
  * Returns SPF_EINVAL for an unknown key or value.
@@ -203,8 +213,10 @@ SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
 
 /*
  * Watchdog.  Every wait on a hardware barrier inside the slicing and matching kernels is bounded
- * (about two seconds of SM clocks): a pipeline that stalls makes its block record a fault and
- * leave through the normal teardown instead of spinning for ever.  spf_check_fault synchronises
+ * (about two seconds of SM clocks): a pipeline that stalls makes its block record a fault, raise the
+ * context's device-global abort flag (every other block gives up at its next poll, blocks that start
+ * later return at entry: one time-out per launch, not one per block), let its in-flight asynchronous
+ * copies and MMAs land, and leave through the normal teardown instead of spinning for ever.  spf_check_fault synchronises
  * `stream`, and returns SPF_EFAULT (text: which kernel, role, block and tile) if any kernel
  * launched through this context since the last check recorded one, else SPF_OK.  The fault is
  * cleared by the call.  spf_orientation_match_host checks it itself before returning.

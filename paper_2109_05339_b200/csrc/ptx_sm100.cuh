@@ -50,13 +50,18 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 // Bounded wait, executed by a whole (converged) warp.  Every wait in libspf is satisfied within
 // microseconds when the pipeline is correct; a wait that lasts SPF_WAIT_CYCLES (about 2 s) means the
 // pipeline is broken, and spinning for ever would take the GPU down with it.  So the wait gives up:
-// it raises the block's abort word in shared memory (every other wait of the block then gives up at
-// its next poll) and returns false.  The caller records the fault in the context's fault word and
-// leaves through the kernel's normal teardown; the host reports SPF_ECUDA at its next check.
+// it raises the block's abort word in shared memory AND the context's device-global abort flag, and
+// returns false.  Every other wait -- of this block through the shared word, of every other block
+// (and of the peer CTA of a pair) through the global flag -- gives up at its next poll, and blocks that
+// start later return at entry (they read the global flag first), so one stalled pipeline costs one
+// time-out, not one per block.  The caller records the fault in the context's fault word and leaves
+// through the kernel's teardown (abort_drain below); the host reports SPF_EFAULT at its next check and
+// clears the flag.
 #ifndef SPF_WAIT_CYCLES
 #define SPF_WAIT_CYCLES (1ll << 32)
 #endif
-__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t *abort_word) {
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t *abort_word,
+                                          volatile uint32_t *global_abort) {
     bool ok = mbar_try_wait(bar, parity);
     if (!ok) {
         const long long t0 = clock64();
@@ -65,11 +70,24 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatil
             if (mbar_try_wait(bar, parity)) { ok = true; break; }
             if ((++polls & 63u) == 0) {
                 if (*abort_word) break;
-                if (clock64() - t0 > SPF_WAIT_CYCLES) { *abort_word = 1u; break; }
+                if ((polls & 1023u) == 0 && *global_abort) { *abort_word = 1u; break; }
+                if (clock64() - t0 > SPF_WAIT_CYCLES) { *abort_word = 1u; *global_abort = 1u; __threadfence(); break; }
             }
         }
     }
     return __all_sync(0xffffffffu, ok);
+}
+// Teardown after an abort: asynchronous work issued before the give-up (bulk tensor copies into this
+// block's shared memory, tcgen05.mma into its TMEM) may still be in flight.  Neither can be cancelled,
+// and both finish within microseconds unless the hardware itself has faulted, so the block simply lets
+// SPF_DRAIN_CYCLES (about 1 ms) pass before it releases TMEM or hands its shared memory to the next
+// block: the fault stays a clean SPF_EFAULT instead of corrupting a neighbour.
+#ifndef SPF_DRAIN_CYCLES
+#define SPF_DRAIN_CYCLES (1ll << 21)
+#endif
+__device__ __forceinline__ void abort_drain() {
+    const long long t0 = clock64();
+    while (clock64() - t0 < SPF_DRAIN_CYCLES) { }
 }
 
 // ---------------------------------------------------------------- TMA
@@ -163,6 +181,16 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
           "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
           "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
           "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+// 32 lanes x 16 consecutive fp32 columns (the epilogue's piece: 16 transient registers)
+__device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
         : "r"(taddr)
         : "memory");
 }

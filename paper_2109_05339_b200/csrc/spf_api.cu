@@ -95,6 +95,9 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     if (!strcmp(key, "force_complex_grid") && (value == 0 || value == 1)) { ctx->opt_force_complex = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_cta_group") && (value == 1 || value == 2)) { ctx->opt_match_cta_group = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_impl") && (value == 0 || value == 1)) { ctx->opt_match_impl = (int)value; return SPF_OK; }
+    if (!strcmp(key, "match_chunk_kblocks") && value >= 0 && value <= (1 << 20)) { ctx->opt_match_chunk_kb = (int)value; return SPF_OK; }
+    if (!strcmp(key, "match_condition") && (value == 0 || value == 1)) { ctx->opt_match_condition = (int)value; return SPF_OK; }
+    if (!strcmp(key, "match_refine") && (value == 0 || value == 1)) { ctx->opt_match_refine = (int)value; return SPF_OK; }
     if (!strcmp(key, "record_events") && (value == 0 || value == 1)) { ctx->opt_record_events = (int)value; return SPF_OK; }
     return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
 }
@@ -106,6 +109,7 @@ int spf_check_fault(spf_ctx *ctx, void *stream_) {
     if (!ctx->h_fault || ctx->h_fault[0] == 0u) return SPF_OK;
     const uint32_t code = ctx->h_fault[0], block = ctx->h_fault[1], unit = ctx->h_fault[2], variant = ctx->h_fault[3];
     ctx->h_fault[0] = ctx->h_fault[1] = ctx->h_fault[2] = ctx->h_fault[3] = 0u;
+    SPF_CUDA(ctx, cudaMemset(ctx->d_abort, 0, sizeof(uint32_t)));   // later launches run again
     if (code >= SPF_FAULT_MATCH) {
         static const char *role[4] = {"TMA producer (slot never freed)", "MMA issuer (accumulator never drained)",
                                       "MMA issuer (operands never arrived)", "epilogue (accumulator never completed)"};

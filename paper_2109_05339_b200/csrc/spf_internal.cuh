@@ -15,6 +15,7 @@
 #define SPF_MAX_W 16
 
 #include "spf_slice_math.cuh"  // SPF_BOX_*: the menu of TMA box sizes (one tensor map per (by, bz) pair)
+#include "spf_match_math.cuh"  // CHUNK_KB: default of option "match_chunk_kblocks"
 
 struct SliceMaps {
     CUtensorMap m[SPF_BOX_N * SPF_BOX_N];  // [iy * SPF_BOX_N + iz]
@@ -33,6 +34,9 @@ struct spf_ctx {
     int opt_match_cta_group = 1;
     int opt_match_impl = 1;       // 1 = CUDA-core difference-form matcher, 0 = tcgen05 GEMM (spf.h)
     int last_match_impl = 1;
+    int opt_match_chunk_kb = spfmm::CHUNK_KB;   // K blocks per accumulator drain of k_match_gemm (0 = whole K)
+    int opt_match_condition = 1;                // 1 = subtract the common vector from the slices (spf_match_math.cuh)
+    int opt_match_refine = 1;                   // 1 = recompute the winner's distance in the difference form
     int gemm_max_clusters[2][2] = {{0, 0}, {0, 0}};  // [CG - 1][NI - 1]: co-resident clusters of k_match_gemm, 0 = not asked yet
     int opt_record_events = 0;
     int64_t launches = 0;
@@ -80,6 +84,9 @@ struct spf_ctx {
     // [0] code (0 = none), [1] block, [2] tile / patch, [3] kernel variant
     volatile uint32_t *h_fault = nullptr;
     uint32_t *d_fault = nullptr;
+    // device-global abort flag (device memory, 1 word): raised by the first pipeline wait that gives up, read by
+    // every block at entry and inside every bounded wait; cleared by spf_check_fault
+    uint32_t *d_abort = nullptr;
 
     std::string err;
 };

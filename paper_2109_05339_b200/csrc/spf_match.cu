@@ -1,18 +1,22 @@
 // libspf: spf_match (steps a6-a8 of SURVEY.md section 8(a)).
 //
-//   d[i][m] = ||I_i||^2 + ||S_m||^2 - 2 I_i . S_m   over unmasked pixels,  best_i = argmin_m d[i][m]
+//   d[i][m] = sum_j (I_ij - S_mj)^2 over unmasked pixels,  best_i = argmin_m d[i][m]
+//           = a_i + b_m - 2 G_im,   a_i = ||I_i - c||^2,  b_m = sum S'_m (S'_m + 2 c),  G_im = I_i . S'_m,  S' = S - c
+// (the conditioned expansion of spf_match_math.cuh: c is one common vector, the mean of up to 1,024 slices).
 //
-// The cross term is a dense contraction (n_img x P) . (M x P)^T and runs on the 5th-generation tensor
+// The cross term G is a dense contraction (n_img x P) . (M x P)^T and runs on the 5th-generation tensor
 // cores: tcgen05.mma with fp32 accumulators in TMEM, operands staged in shared memory by TMA.
 // fp32-equivalent products come from a two-term fp16 split of each operand, x * 2^e = h1 + h2 (+ <=2^-22
 // relative), after a power-of-two rescale into fp16 range.  Photon-count images are exact in ONE fp16
 // term (integers < 2048), which is tested on the device: the kernel instantiated for one image plane
 // issues 2 products per K step (I1.S1, I1.S2), the one for two planes issues 3 (adds I2.S1).  Both
 // instantiations are launched and the one the data does not need returns at once, so the host never
-// synchronises.  The epilogue reads the accumulator tile out of TMEM, adds the norms and keeps a
-// running (min, argmin) per image row; tiles merge through a 64-bit atomicMin on
+// synchronises.  The epilogue reads the accumulator tile out of TMEM, adds a_i + b_m (fp64, rounded once)
+// and keeps a running (min, argmin) per image row; tiles merge through a 64-bit atomicMin on
 // (order-preserving bits of d) << 32 | m, so the lowest index wins exact ties and the distance
-// matrix never exists in memory.
+// matrix never exists in memory.  k_match_refine then recomputes each winner's distance in the
+// difference form, so best_dist carries no cancellation error of the expansion.
+#include <assert.h>
 #include <cuda_fp16.h>
 #include <math.h>
 
@@ -29,7 +33,7 @@ using spfmm::A_TILE_BYTES;
 constexpr int EPI_WARPS = 8;                      // two per TMEM lane quadrant, each takes one half of the tile's columns
 constexpr int GEMM_THREADS = 64 + 32 * EPI_WARPS; // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-9 epilogue
 constexpr int EPI_COLS = BN / (EPI_WARPS / 4);    // 128 accumulator registers per epilogue thread
-using spfmm::CHUNK_KB;
+constexpr int EPI_PIECE = 16;                     // columns per tcgen05.ld (16 transient registers beside the 128 running sums)
 constexpr int ACC_STAGES = 2;
 constexpr int TMEM_COLS = ACC_STAGES * BN;        // 512: all of TMEM, one CTA per SM
 constexpr size_t SMEM_AUX = spfmm::SMEM_AUX;
@@ -49,15 +53,17 @@ struct GemmCfg {
 struct MatchArgs {
     int64_t n_img, M;
     int kblocks;            // P_pad / 64
+    int chunk_kb;           // K blocks accumulated in TMEM between two drains by the epilogue (>= 1)
     int n_ib, n_mb;         // tiles along images / slices
     unsigned long long *keys;
-    const float *nI, *nS;
+    const double *aI, *bS;  // a_i = ||I_i - c||^2, b_m = sum S'_m (S'_m + 2 c)
     const uint32_t *scal;   // [2] = image plane 2 needed, [4] = eI, [5] = eS
-    uint32_t *fault;        // context fault word (host-mapped): written when a pipeline wait gives up
+    uint32_t *fault;        // context fault record (host-mapped): written when a pipeline wait gives up
+    uint32_t *abort_flag;   // context abort flag (device memory): set by the first wait that gives up, read by every block
 };
 
 struct WsLayout {
-    size_t scal, keys, nI, nS, planesI, planesS, total;
+    size_t scal, keys, aI, bS, common, planesI, planesS, total;
     int64_t Ppad;
 };
 
@@ -69,8 +75,9 @@ WsLayout ws_layout(int64_t n_img, int64_t M, int64_t P) {
     size_t off = 0;
     L.scal = off; off += 1024;
     L.keys = off; off += rup((size_t)n_img * 8, 1024);
-    L.nI = off; off += rup((size_t)n_img * 4, 1024);
-    L.nS = off; off += rup((size_t)M * 4, 1024);
+    L.aI = off; off += rup((size_t)n_img * 8, 1024);
+    L.bS = off; off += rup((size_t)M * 8, 1024);
+    L.common = off; off += rup((size_t)L.Ppad * 4, 1024);
     L.planesI = off; off += rup((size_t)2 * n_img * L.Ppad * 2, 1024);
     L.planesS = off; off += rup((size_t)2 * M * L.Ppad * 2, 1024);
     L.total = off;
@@ -80,25 +87,51 @@ WsLayout ws_layout(int64_t n_img, int64_t M, int64_t P) {
 // ------------------------------------------------------------------------------------------
 // a6 + operand preparation
 // ------------------------------------------------------------------------------------------
-// max |x| over unmasked pixels, as the bit pattern of a non-negative float (orders like an unsigned)
-__global__ void k_absmax(const float *__restrict__ x, int64_t rows, int64_t P, const uint8_t *__restrict__ mask,
-                         uint32_t *__restrict__ out) {
+// c[j] = mean over the rows 0, step, 2 step, ... of the slices (fp32 sum in ascending row order), 0 in masked
+// pixels; one thread per pixel, so a warp reads 128 consecutive bytes of every row it visits.  condition = 0
+// leaves c = 0 (the plain expansion; option "match_condition").  c is [Ppad]; the K padding is zeroed by the caller.
+__global__ void k_common_vector(const float *__restrict__ slices, int64_t M, int64_t P, const uint8_t *__restrict__ mask,
+                                int condition, float *__restrict__ c) {
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= P) return;
+    float v = 0.0f;
+    if (condition && (!mask || mask[j])) {
+        const int64_t step = spfmm::common_step((long)M);
+        float sum = 0.0f;
+        for (int64_t m = 0; m < M; m += step) sum += slices[m * P + j];
+        v = sum * (1.0f / (float)spfmm::common_count((long)M));
+    }
+    c[j] = v;
+}
+
+// max |x| (which = 0, images) or max |x - c| (which = 1, slices) over unmasked pixels, as the bit pattern of a
+// non-negative float (orders like an unsigned).  Blocks stride over rows, threads over the pixels of a row:
+// no integer division or modulo per element, coalesced loads.
+__global__ void __launch_bounds__(256) k_absmax(const float *__restrict__ x, int64_t rows, int64_t P,
+                                                const uint8_t *__restrict__ mask, const float *__restrict__ c, int which,
+                                                uint32_t *__restrict__ out) {
     uint32_t m = 0;
-    const int64_t total = rows * P;
-    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
-        if (mask && !mask[idx % P]) continue;
-        m = max(m, __float_as_uint(fabsf(x[idx])));
+    for (int64_t r = blockIdx.x; r < rows; r += gridDim.x) {
+        const float *xr = x + r * P;
+        for (int64_t j = threadIdx.x; j < P; j += blockDim.x) {
+            if (mask && !mask[j]) continue;
+            const float v = which ? spfmm::conditioned(xr[j], c[j]) : xr[j];
+            m = max(m, __float_as_uint(fabsf(v)));
+        }
     }
     m = __reduce_max_sync(0xffffffffu, m);
     if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
 }
 
-// One block per row: x * 2^e = h1 + h2 as two fp16 planes (zero in masked pixels and in the K padding),
-// ||x||^2 over unmasked pixels accumulated in fp64, and (images) the running-argmin key reset.
-// which = 0: images (sets scal[2] when some residual is non-zero, resets keys), 1: slices.
+// One block per row: v * 2^e = h1 + h2 as two fp16 planes (zero in masked pixels and in the K padding), where
+//   which = 0 (images): v = the RAW value,   term = a_i = sum (x - c)^2; sets scal[2] when some residual is
+//                       non-zero and resets the running-argmin key;
+//   which = 1 (slices): v = S' = fl(x - c),  term = b_m = sum S' (S' + 2 c);
+// both sums over unmasked pixels, accumulated in fp64.
 __global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int64_t P, int64_t Ppad,
-                                               const uint8_t *__restrict__ mask, uint32_t *__restrict__ scal, int which,
-                                               int64_t rows, __half *__restrict__ planes, float *__restrict__ norms,
+                                               const uint8_t *__restrict__ mask, const float *__restrict__ c,
+                                               uint32_t *__restrict__ scal, int which, int64_t rows,
+                                               __half *__restrict__ planes, double *__restrict__ term,
                                                unsigned long long *__restrict__ keys) {
     const int64_t row = blockIdx.x;
     const int e = spfmm::scale_exponent(scal[which]);
@@ -107,14 +140,17 @@ __global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int6
     __half *h1 = planes + row * Ppad, *h2 = planes + (rows + row) * Ppad;
     double acc = 0.0;
     bool inexact = false;
-    for (int64_t c = threadIdx.x; c < Ppad; c += blockDim.x) {
+    for (int64_t j = threadIdx.x; j < Ppad; j += blockDim.x) {
         float v = 0.0f;
-        if (c < P && (!mask || mask[c])) v = xr[c];
-        acc += (double)v * (double)v;
+        if (j < P && (!mask || mask[j])) {
+            const float raw = xr[j], cj = c[j];
+            if (which) { v = spfmm::conditioned(raw, cj); acc += spfmm::slice_term(v, cj); }
+            else { v = raw; acc += spfmm::image_term(raw, cj); }
+        }
         uint16_t a, b;
         inexact |= spfmm::split_fp16(v, sc, a, b);
-        h1[c] = __ushort_as_half(a);
-        h2[c] = __ushort_as_half(b);
+        h1[j] = __ushort_as_half(a);
+        h2[j] = __ushort_as_half(b);
     }
     __shared__ double red[8];
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -127,7 +163,7 @@ __global__ void __launch_bounds__(256) k_split(const float *__restrict__ x, int6
     if (threadIdx.x == 0) {
         double s = 0.0;
         for (int k = 0; k < (int)(blockDim.x >> 5); ++k) s += red[k];
-        norms[row] = (float)s;
+        term[row] = s;
         if (which == 0) keys[row] = ~0ull;
         if (row == 0) scal[4 + which] = (uint32_t)e;
     }
@@ -142,6 +178,34 @@ __global__ void k_match_finalize(const unsigned long long *__restrict__ keys, in
     best_dist[i] = (k == ~0ull) ? __uint_as_float(0x7fc00000u) : spfmm::unorderable((uint32_t)(k >> 32));
 }
 
+// The winner's distance by the definition: d = sum_j (I_ij - S_mj)^2 over unmasked pixels, differences
+// and sum in fp64, rounded once.  One block per image; n_img x P pixel pairs in all (1e-4 of the contraction's work).
+// The tensor-core pass decides WHICH orientation wins; this makes the reported distance free of the expansion's
+// cancellation.  Rows with no winner (index -1) keep their NaN.
+__global__ void __launch_bounds__(256) k_match_refine(const float *__restrict__ images, const float *__restrict__ slices,
+                                                      int64_t M, int64_t P, const uint8_t *__restrict__ mask,
+                                                      const int32_t *__restrict__ best_idx, float *__restrict__ best_dist) {
+    const int64_t i = blockIdx.x;
+    const int64_t m = best_idx[i];
+    if (m < 0 || m >= M) return;
+    const float *I = images + i * P, *S = slices + m * P;
+    double acc = 0.0;
+    for (int64_t j = threadIdx.x; j < P; j += blockDim.x) {
+        if (mask && !mask[j]) continue;
+        const double t = (double)I[j] - (double)S[j];
+        acc += t * t;
+    }
+    __shared__ double red[8];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) s += red[k];
+        best_dist[i] = (float)s;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // a7 + a8: tcgen05 GEMM with the fused norm-add / argmin epilogue
 // ------------------------------------------------------------------------------------------
@@ -151,8 +215,11 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
              const __grid_constant__ CUtensorMap mapB0, const __grid_constant__ CUtensorMap mapB1, const MatchArgs a) {
     using Cfg = GemmCfg<CG, NI>;
     constexpr int ST = Cfg::STAGES;
-    // the instantiation the data does not need leaves before touching any barrier or TMEM
+    // the instantiation the data does not need leaves before touching any barrier or TMEM; so does every block
+    // once some block's pipeline has given up (both conditions are uniform over a CTA pair)
     if ((a.scal[2] != 0u) != (NI == 2)) return;
+    volatile uint32_t *g_abort = a.abort_flag;
+    if (*g_abort) return;
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;  // SWIZZLE_128B tiles need 1024-byte alignment
@@ -161,8 +228,18 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     uint8_t *aux_p = smem_al + (size_t)ST * Cfg::STAGE_BYTES;
     const uint32_t bar_full = aux, bar_empty = aux + 8 * ST, bar_tfull = aux + 16 * ST, bar_tempty = bar_tfull + 8 * ACC_STAGES;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(aux_p + 16 * ST + 16 * ACC_STAGES);
-    volatile uint32_t *abort_w = tmem_slot + 1;              // raised by the first wait that gives up
-    float *nsbuf = reinterpret_cast<float *>(aux_p + 1024);  // [EPI_WARPS][EPI_COLS]
+    volatile uint32_t *abort_w = tmem_slot + 1;              // raised by the first wait of this block that gives up
+    static_assert(16 * 6 + 16 * ACC_STAGES + 8 <= (int)SMEM_AUX, "barriers, TMEM slot and abort word fit the auxiliary block");
+#ifdef SPF_DEBUG
+    // invariants the descriptors and the bulk copies rely on (table of PTX wrappers)
+    if (threadIdx.x == 0) {
+        assert((smem_base & 1023u) == 0u);                                           // SWIZZLE_128B atom alignment
+        assert(smem_base + ST * Cfg::STAGE_BYTES + SMEM_AUX <= ptx::smem_u32(smem_raw) + (uint32_t)Cfg::SMEM_BYTES);
+        assert(((smem_base + ST * Cfg::STAGE_BYTES) >> 4) < (1u << 14));            // 14-bit start-address field of the UMMA descriptor
+        assert((bar_full & 7u) == 0u);
+        assert(gridDim.x % CG == 0 && a.chunk_kb >= 1);
+    }
+#endif
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
@@ -183,6 +260,9 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     if (CG == 2) ptx::cluster_sync(); else __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+#ifdef SPF_DEBUG
+    if (threadIdx.x == 0) assert((tmem_base & 0xffffu) + TMEM_COLS <= 512u && (tmem_base >> 16) == 0u);   // whole TMEM, lane 0
+#endif
 
     auto tile_coords = [&](int t, int &ib, int &mb) { spfmm::tile_coords(t, a.n_ib, a.n_mb, ib, mb); };
 
@@ -204,7 +284,7 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
             const int rowA = ib * (TILE_ROWS * CG) + (int)rank * TILE_ROWS;
             const int rowB = mb * BN + (int)rank * Cfg::B_ROWS;
             for (int kb = 0; kb < a.kblocks; ++kb) {
-                if (!ptx::mbar_wait(bar_empty + 8 * s, ph ^ 1u, abort_w)) { give_up(0, t); alive = false; break; }
+                if (!ptx::mbar_wait(bar_empty + 8 * s, ph ^ 1u, abort_w, g_abort)) { give_up(0, t); alive = false; break; }
                 if (lane == 0) {
                     const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
                     const uint32_t fb = bar_full + 8 * s;
@@ -234,16 +314,16 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
             int s = 0; uint32_t ph = 0; int as = 0; uint32_t aph = 0;
             bool alive = true;
             for (int t = cluster_id; alive && t < n_tiles; t += n_clusters) {
-                // K runs in chunks of CHUNK_KB blocks; each chunk starts on a cleared accumulator stage
+                // K runs in chunks of a.chunk_kb blocks; each chunk starts on a cleared accumulator stage
                 // and is handed to the epilogue warps, which keep the running sum (spf_match_math.cuh)
-                for (int kb0 = 0; alive && kb0 < a.kblocks; kb0 += CHUNK_KB) {
+                for (int kb0 = 0; alive && kb0 < a.kblocks; kb0 += a.chunk_kb) {
                     // epilogue has drained this accumulator stage
-                    if (!ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u, abort_w)) { give_up(1, t); alive = false; break; }
+                    if (!ptx::mbar_wait(bar_tempty + 8 * as, aph ^ 1u, abort_w, g_abort)) { give_up(1, t); alive = false; break; }
                     ptx::tc_fence_after();
                     const uint32_t tacc = tmem_base + (uint32_t)(as * BN);
-                    const int kend = min(kb0 + CHUNK_KB, a.kblocks);
+                    const int kend = min(kb0 + a.chunk_kb, a.kblocks);
                     for (int kb = kb0; kb < kend; ++kb) {
-                        if (!ptx::mbar_wait(bar_full + 8 * s, ph, abort_w)) { give_up(2, t); alive = false; break; }
+                        if (!ptx::mbar_wait(bar_full + 8 * s, ph, abort_w, g_abort)) { give_up(2, t); alive = false; break; }
                         ptx::tc_fence_after();
                         if (lane == 0) {
                             const uint32_t st = smem_base + s * Cfg::STAGE_BYTES;
@@ -269,40 +349,35 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
             }
         }
     } else {
-        // ===================== epilogue: TMEM chunks -> fp32 registers -> norm add + running argmin =====================
+        // ===================== epilogue: TMEM chunks -> fp32 registers -> a_i + b_m - 2 G, running argmin =====================
         // Warp (warp - 2) reads TMEM lane quadrant warp % 4 (the only one the hardware lets it read) and
         // the column half (warp - 2) / 4 of the tile: thread = one image row x EPI_COLS slices, whose
         // cross terms it sums chunk by chunk in registers (round to nearest).  Each warp works alone --
-        // its own lanes, its own copy of its ||S||^2 values -- so epilogue warps never wait for one another.
+        // its own lanes, nothing shared -- so epilogue warps never wait for one another.
         const int ew = warp - 2;
         const int q = warp & 3;                 // TMEM lane quadrant
         const int col0 = (ew >> 2) * EPI_COLS;  // first tile column of this warp
-        float *nsb = nsbuf + ew * EPI_COLS;
         const float neg2sc = spfmm::cross_scale((int)a.scal[4], (int)a.scal[5]);
         int as = 0; uint32_t aph = 0;
         bool alive = true;
         for (int t = cluster_id; alive && t < n_tiles; t += n_clusters) {
             int ib, mb; tile_coords(t, ib, mb);
             const int64_t m0 = (int64_t)mb * BN + col0;
-            __syncwarp();
-            for (int k = lane; k < EPI_COLS; k += 32) nsb[k] = (m0 + k < a.M) ? a.nS[m0 + k] : INFINITY;
-            __syncwarp();
             const int64_t i = (int64_t)ib * (TILE_ROWS * CG) + (int64_t)rank * TILE_ROWS + q * 32 + lane;
-            const float nIv = (i < a.n_img) ? a.nI[i] : 0.0f;
             float acc[EPI_COLS];
 #pragma unroll
             for (int k = 0; k < EPI_COLS; ++k) acc[k] = 0.0f;
-            for (int kb0 = 0; kb0 < a.kblocks; kb0 += CHUNK_KB) {
-                if (!ptx::mbar_wait(bar_tfull + 8 * as, aph, abort_w)) { give_up(3, t); alive = false; break; }
+            for (int kb0 = 0; kb0 < a.kblocks; kb0 += a.chunk_kb) {
+                if (!ptx::mbar_wait(bar_tfull + 8 * as, aph, abort_w, g_abort)) { give_up(3, t); alive = false; break; }
                 ptx::tc_fence_after();
                 const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * BN + col0);
 #pragma unroll
-                for (int c = 0; c < EPI_COLS / 32; ++c) {
-                    uint32_t r[32];
-                    ptx::tmem_ld_32x32(trow + c * 32, r);
+                for (int c = 0; c < EPI_COLS / EPI_PIECE; ++c) {
+                    uint32_t r[EPI_PIECE];
+                    ptx::tmem_ld_32x16(trow + c * EPI_PIECE, r);
                     ptx::tmem_ld_wait();
 #pragma unroll
-                    for (int k = 0; k < 32; ++k) acc[c * 32 + k] += __uint_as_float(r[k]);
+                    for (int k = 0; k < EPI_PIECE; ++k) acc[c * EPI_PIECE + k] += __uint_as_float(r[k]);
                 }
                 ptx::tc_fence_before();
                 __syncwarp();
@@ -310,19 +385,27 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
                 if (++as == ACC_STAGES) { as = 0; aph ^= 1u; }
             }
             if (!alive) break;
-            float best = INFINITY; uint32_t bm = 0xffffffffu;
+            if (i < a.n_img) {
+                // once per pair per tile: fp64 add of the two row terms and the (exactly rescaled) cross term
+                const double aIv = a.aI[i];
+                float best = INFINITY; uint32_t bm = 0xffffffffu;
 #pragma unroll
-            for (int k = 0; k < EPI_COLS; ++k) {
-                const float d = spfmm::distance(nIv, nsb[k], neg2sc, acc[k]);
-                if (d < best) { best = d; bm = (uint32_t)(m0 + k); }
+                for (int k = 0; k < EPI_COLS; ++k) {
+                    if (m0 + k < a.M) {
+                        const float d = spfmm::distance(aIv, __ldg(a.bS + m0 + k), neg2sc, acc[k]);
+                        if (d < best) { best = d; bm = (uint32_t)(m0 + k); }   // ascending k: the lowest index wins ties
+                    }
+                }
+                if (bm != 0xffffffffu) atomicMin(&a.keys[i], spfmm::pack_key(best, bm));
             }
-            if (i < a.n_img && bm != 0xffffffffu)
-                atomicMin(&a.keys[i], spfmm::pack_key(best, bm));
         }
     }
 
+    // teardown.  After a give-up, bulk copies and MMAs issued earlier may still be in flight: let them land
+    // before TMEM is released and the shared memory goes to the next block (ptx::abort_drain).
     ptx::tc_fence_before();
     if (CG == 2) ptx::cluster_sync(); else __syncthreads();
+    if (*abort_w || *g_abort) ptx::abort_drain();
     if (warp == 1) ptx::tmem_dealloc<CG>(tmem_base, TMEM_COLS);
 }
 
@@ -521,7 +604,8 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     uint8_t *ws = (uint8_t *)workspace;
     uint32_t *scal = (uint32_t *)(ws + L.scal);
     unsigned long long *keys = (unsigned long long *)(ws + L.keys);
-    float *nI = (float *)(ws + L.nI), *nS = (float *)(ws + L.nS);
+    double *aI = (double *)(ws + L.aI), *bS = (double *)(ws + L.bS);
+    float *cvec = (float *)(ws + L.common);
     __half *plI = (__half *)(ws + L.planesI), *plS = (__half *)(ws + L.planesS);
 
     int rc;
@@ -543,14 +627,18 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
         SPF_LAUNCH_CHECK(ctx);
         return SPF_OK;
     }
+    // a6: common vector, abs-max of both operands (images raw, slices minus c), two-term fp16 split, a_i and b_m
+    SPF_CUDA(ctx, cudaMemsetAsync(cvec, 0, (size_t)L.Ppad * 4, st));
+    k_common_vector<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(slices, M, P, mask, ctx->opt_match_condition, cvec);
+    SPF_LAUNCH_CHECK(ctx);
     const int rb = ctx->sm_count * 8;
-    k_absmax<<<rb, 256, 0, st>>>(images, n_img, P, mask, scal + 0);
+    k_absmax<<<(unsigned)(n_img < rb ? n_img : rb), 256, 0, st>>>(images, n_img, P, mask, cvec, 0, scal + 0);
     SPF_LAUNCH_CHECK(ctx);
-    k_absmax<<<rb, 256, 0, st>>>(slices, M, P, mask, scal + 1);
+    k_absmax<<<(unsigned)(M < rb ? M : rb), 256, 0, st>>>(slices, M, P, mask, cvec, 1, scal + 1);
     SPF_LAUNCH_CHECK(ctx);
-    k_split<<<(unsigned)n_img, 256, 0, st>>>(images, P, L.Ppad, mask, scal, 0, n_img, plI, nI, keys);
+    k_split<<<(unsigned)n_img, 256, 0, st>>>(images, P, L.Ppad, mask, cvec, scal, 0, n_img, plI, aI, keys);
     SPF_LAUNCH_CHECK(ctx);
-    k_split<<<(unsigned)M, 256, 0, st>>>(slices, P, L.Ppad, mask, scal, 1, M, plS, nS, nullptr);
+    k_split<<<(unsigned)M, 256, 0, st>>>(slices, P, L.Ppad, mask, cvec, scal, 1, M, plS, bS, nullptr);
     SPF_LAUNCH_CHECK(ctx);
 
     const int CG = ctx->opt_match_cta_group;
@@ -563,7 +651,8 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     args.n_img = n_img; args.M = M; args.kblocks = (int)(L.Ppad / BK);
     args.n_ib = (int)((n_img + TILE_ROWS * CG - 1) / (TILE_ROWS * CG));
     args.n_mb = (int)((M + BN - 1) / BN);
-    args.keys = keys; args.nI = nI; args.nS = nS; args.scal = scal; args.fault = ctx->d_fault;
+    args.chunk_kb = ctx->opt_match_chunk_kb > 0 ? ctx->opt_match_chunk_kb : args.kblocks;   // 0 = the whole of K in TMEM
+    args.keys = keys; args.aI = aI; args.bS = bS; args.scal = scal; args.fault = ctx->d_fault; args.abort_flag = ctx->d_abort;
     if ((int64_t)args.n_ib * args.n_mb > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: too many tiles");
     if ((rc = spf_record_event(ctx, 2, st))) return rc;
     if (CG == 2) {
@@ -578,6 +667,10 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     ctx->ev_valid[1] = ctx->ev_valid[2] = ctx->opt_record_events != 0;
     k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
     SPF_LAUNCH_CHECK(ctx);
+    if (ctx->opt_match_refine) {
+        k_match_refine<<<(unsigned)n_img, 256, 0, st>>>(images, slices, M, P, mask, best_idx, best_dist);
+        SPF_LAUNCH_CHECK(ctx);
+    }
     return SPF_OK;
 }
 

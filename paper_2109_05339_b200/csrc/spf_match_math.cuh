@@ -5,7 +5,20 @@
 // accumulation, norm add, packed argmin keys) against the oracle.  It is NOT a CPU fallback: nothing
 // in the library's ABI reaches the host versions.
 //
-//   d[i][m] = ||I_i||^2 + ||S_m||^2 - 2 I_i . S_m,   I_i . S_m = 2^-(eI+eS) (I1 + I2) . (S1 + S2)
+// Conditioned expansion (SURVEY.md section 7 "Split precision vs cancellation").  With one
+// common vector c (the mean of up to 1,024 evenly spaced slices; any c gives the same d in exact arithmetic) and
+// S'_m = fl(S_m - c):
+//   d[i][m] = sum_j (I_ij - S_mj)^2 = sum_j ((I_ij - c_j) - S'_mj)^2 = a_i + b_m - 2 G_im
+//   a_i  = sum_j (I_ij - c_j)^2                 per image, fp64
+//   b_m  = sum_j S'_mj (S'_mj + 2 c_j)          per slice, fp64   ( = ||S'||^2 + 2 c . S' )
+//   G_im = sum_j I_ij S'_mj                     the contraction (tensor cores); the images stay RAW, so photon
+//                                               counts remain exact in one fp16 plane
+// Everything the slices have in common (the radial fall-off of a diffraction pattern) is gone from G, so the
+// terms that cancel are the size of ||I - c||^2 + ||S'||^2, not of ||I||^2 + ||S||^2, and the accumulator's
+// rounding acts on a signed sum instead of a monotone one.  a_i + b_m - 2 G is added in fp64 (once per pair per
+// tile: free), and the winner's distance is recomputed in the difference form (k_match_refine) so that best_dist
+// never carries the expansion's cancellation error.
+//   I_i . S'_m = 2^-(eI+eS) (I1 + I2) . (S1 + S2)
 //   x 2^e = h1 + h2 + r,  h1 = fp16(x 2^e), h2 = fp16(x 2^e - h1), |r| <= 2^-22 |x 2^e| (or 2^-25 absolute)
 //   products kept: I1.S1 + I1.S2 (+ I2.S1 when some image value is not exact in one fp16 term)
 #pragma once
@@ -26,18 +39,26 @@ constexpr int BN = 256;         // slices per tile (UMMA N)
 constexpr int TILE_ROWS = 128;  // image rows per CTA (UMMA M = 128 * CG)
 constexpr int TILE_GROUP = 8;   // image blocks whose tiles are scheduled together (L2 reuse of slice rows)
 // K blocks summed inside the tensor core's accumulator (TMEM) before the epilogue warps add that chunk
-// to their own fp32 registers with round-to-nearest FADDs.  Tensor-core accumulators have been measured
-// to round toward zero on earlier generations; over K = 65,536 that is a bias of ~1e-4 of the cross
-// term, i.e. up to 1e-3 of the distance (tests/test_hostsim_match.py reproduces it), ten times the parity
-// bar.  With chunks of 4 x 64 the bias stays below 2e-5 of the distance under either rounding.
-constexpr int CHUNK_KB = 4;
+// to their own fp32 registers with round-to-nearest FADDs (run-time option "match_chunk_kblocks"; this is its
+// default, 0 = the whole of K in TMEM).  Tensor-core accumulators have been measured to round toward zero on
+// earlier generations; whether sm_100a's do is not known yet (no hardware run), so the default is chosen from
+// the CPU replay under BOTH roundings (tests/test_hostsim_match.py, Paper-scale statistics, P = 65,536, worst
+// relative error of any winning distance before k_match_refine):
+//   truncating accumulator, conditioned:  whole K 1.9e-4 | 64 blocks 1.8e-5 | 4 blocks 1.6e-6
+//   truncating accumulator, plain:        whole K 3.7e-4 | 64 blocks 3.2e-5 | 4 blocks 6.1e-6
+//   round to nearest (either form):       <= 5e-6 at any chunk size
+// 32 blocks (2,048 pixels) keeps the truncating case an order of magnitude inside the 1e-4 bar and drains the
+// 128 x 256 accumulator 32 times per tile at P = 65,536 (it was 256 times at the round-1 value of 4): one drain
+// (128 KB of TMEM reads) per 32,768 tensor-pipe cycles, hidden behind the other accumulator stage.
+constexpr int CHUNK_KB = 32;
+constexpr int COMMON_ROWS = 1024;   // slices averaged into the common vector c (evenly spaced over M)
 
 // ---------------------------------------------------------------- shared-memory stage layout
 // One pipeline stage of CTA `rank` of a CG-CTA group holds, in this order: NI image tiles
 // (TILE_ROWS x BK fp16 each: plane 1, then plane 2 when NI == 2), then the two slice tiles
 // (BN / CG rows x BK fp16 each: plane 1, plane 2).  Every tile is a multiple of 1024 bytes.
 constexpr int A_TILE_BYTES = TILE_ROWS * BK * 2;   // 16 KB
-constexpr int SMEM_AUX = 6144;                     // 1 KB barriers + tmem pointer + abort word; 4 KB per-warp ||S||^2 tiles
+constexpr int SMEM_AUX = 1024;                     // barriers + tmem pointer + abort word
 constexpr int SMEM_BUDGET = 227 * 1024;
 constexpr int b_rows(int cg) { return BN / cg; }
 constexpr int b_tile_bytes(int cg) { return b_rows(cg) * BK * 2; }
@@ -117,11 +138,22 @@ SPF_MHD bool split_fp16(float x, float sc, uint16_t &h1, uint16_t &h2) {
     return r != 0.0f;
 }
 
+// ---------------------------------------------------------------- a6: conditioning
+// rows of the slice array averaged into c: m = 0, step, 2 step, ... (at most COMMON_ROWS of them)
+SPF_MHD long common_step(long M) { return M <= COMMON_ROWS ? 1 : (M + COMMON_ROWS - 1) / COMMON_ROWS; }
+SPF_MHD long common_count(long M) { const long st = common_step(M); return (M + st - 1) / st; }
+// the conditioned slice value S' = fl(S - c), one fp32 subtraction; everything downstream (planes, b_m) uses S'
+SPF_MHD float conditioned(float s, float c) { return s - c; }
+// per-pixel terms of a_i and b_m (fp64)
+SPF_MHD double image_term(float x, float c) { const double t = (double)x - (double)c; return t * t; }
+SPF_MHD double slice_term(float sp, float c) { return (double)sp * ((double)sp + 2.0 * (double)c); }
+
 // ---------------------------------------------------------------- a8: epilogue
 // factor that undoes both rescales and carries the -2 of the cross term
 SPF_MHD float cross_scale(int eI, int eS) { return ldexpf(-2.0f, -(eI + eS)); }
 
-SPF_MHD float distance(float nI, float nS, float neg2sc, float acc) { return nI + fmaf(neg2sc, acc, nS); }
+// d = a_i + b_m - 2 G in fp64, rounded once; neg2sc * acc is exact in fp32 (a power-of-two scaling)
+SPF_MHD float distance(double aI, double bS, float neg2sc, float acc) { return (float)(aI + bS + (double)(neg2sc * acc)); }
 
 // fp32 -> uint32 that orders like the float (negative values below positive ones)
 SPF_MHD uint32_t orderable(float d) {

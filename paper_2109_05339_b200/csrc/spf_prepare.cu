@@ -95,7 +95,7 @@ void spf_destroy(spf_ctx *ctx) {
     cudaSetDevice(ctx->prm.device);
     if (ctx->plan_ok) cufftDestroy(ctx->plan);
     cudaFree(ctx->d_deapod); cudaFree(ctx->d_fft); cudaFree(ctx->d_gridc); cudaFree(ctx->d_gridr);
-    cudaFree(ctx->d_flag); cudaFree(ctx->d_patch);
+    cudaFree(ctx->d_flag); cudaFree(ctx->d_patch); cudaFree(ctx->d_abort);
     if (ctx->h_fault) cudaFreeHost((void *)ctx->h_fault);
     auto &b = ctx->hb;
     cudaFree(b.model); cudaFree(b.quats); cudaFree(b.pix); cudaFree(b.images); cudaFree(b.slices);
@@ -150,6 +150,8 @@ static int create_impl(spf_ctx *ctx, const spf_params *p) {
     memset(hf, 0, 4 * sizeof(uint32_t));
     ctx->h_fault = (volatile uint32_t *)hf;
     SPF_CUDA(ctx, cudaHostGetDevicePointer((void **)&ctx->d_fault, hf, 0));
+    SPF_CUDA(ctx, cudaMalloc(&ctx->d_abort, sizeof(uint32_t)));
+    SPF_CUDA(ctx, cudaMemset(ctx->d_abort, 0, sizeof(uint32_t)));
     cufftResult fr = cufftPlan3d(&ctx->plan, ctx->nf, ctx->nf, ctx->nf, CUFFT_C2C);
     if (fr != CUFFT_SUCCESS) return spf_set_err(ctx, fr == CUFFT_ALLOC_FAILED ? SPF_ENOMEM : SPF_ECUDA, "cufftPlan3d(%d^3) failed: %d", ctx->nf, (int)fr);
     ctx->plan_ok = true;

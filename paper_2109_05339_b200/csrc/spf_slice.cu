@@ -38,7 +38,8 @@ struct SliceArgs {
     double inv_nf;
     float beta;
     uint32_t cap_bytes;     // dynamic shared memory available for the tile
-    uint32_t *fault;        // context fault word (host-mapped): written when the tile wait gives up
+    uint32_t *fault;        // context fault record (host-mapped): written when the tile wait gives up
+    uint32_t *abort_flag;   // context abort flag (device memory): set by the first wait that gives up, read by every block
     float coef[SPF_MAX_W][SPF_MAX_DEG + 1];  // phi at tap t as a polynomial in u = 2 (f + w/2) - 1
     SliceMaps maps;
 };
@@ -128,6 +129,8 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
     constexpr int CELL = 4 * E;                // bytes per cell
     const int w = W ? W : a.w;
     const int tid = threadIdx.x;
+    // one stalled tile costs one time-out, not one per block: blocks that start after a give-up leave at once
+    if (STAGED && *reinterpret_cast<volatile uint32_t *>(a.abort_flag)) return;
     const int64_t m = blockIdx.x / a.n_patches;
     const int64_t patch = blockIdx.x - m * a.n_patches;
 
@@ -219,12 +222,13 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         __syncwarp();
     }
     if (STAGED && staged) {
-        if (!ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort)) {
+        if (!ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort, a.abort_flag)) {
             if (tid == 0) {
                 a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)patch; a.fault[3] = (uint32_t)(W * 10 + (REAL ? 1 : 0) + 100 * IMPL);
                 a.fault[0] = SPF_FAULT_SLICE;
                 __threadfence_system();
             }
+            ptx::abort_drain();   // bulk copies still in flight must land before this shared memory goes to the next block
             return;
         }
         const float *tile = reinterpret_cast<const float *>(s_tile);
@@ -348,7 +352,7 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.beta = (float)ctx->beta;
     args.deg = spfm::fit_kernel_polys(ctx->w, ctx->beta, args.coef);
     args.maps = real ? ctx->maps_r : ctx->maps_c;
-    args.fault = ctx->d_fault;
+    args.fault = ctx->d_fault; args.abort_flag = ctx->d_abort;
     const int impl = ctx->opt_slice_impl;
     if ((impl == IMPL_STAGED || impl == IMPL_COOP) && !ctx->maps_ok)
         return spf_set_err(ctx, SPF_ECUDA, "spf_slice: slice_impl %d needs the TMA tensor maps, which could not be encoded: %s", impl,

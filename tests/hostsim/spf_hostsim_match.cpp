@@ -3,8 +3,10 @@
 // product loads this library and it is not a CPU fallback.
 //
 // What is replayed, kernel by kernel (spf_match.cu):
+//   k_common_vector       c = mean of up to 1,024 evenly spaced slices (the conditioning vector)
 //   k_absmax / k_split    abs-max over unmasked pixels -> power-of-two rescale -> two fp16 planes per
-//                         operand (zero in masked pixels and in the K padding), fp64-accumulated norms
+//                         operand (raw images; slices minus c; zero in masked pixels and in the K padding),
+//                         fp64-accumulated a_i = sum (I - c)^2 and b_m = sum S' (S' + 2 c)
 //   k_match_gemm          persistent tile loop (tile_coords, cluster stride), per K block the TMA boxes
 //                         of every CTA of the group written into a byte image of its shared-memory
 //                         stage (128-byte swizzle, zero fill outside the tensor), the tcgen05.mma
@@ -12,6 +14,7 @@
 //                         fp32 accumulation product by product in issue order, the epilogue's norm add
 //                         and running argmin per TMEM lane, packed 64-bit keys merged with min
 //   k_match_finalize      key -> (index, distance)
+//   k_match_refine        the winner's distance recomputed as sum (I - S)^2
 // What is NOT modelled: the tensor core's internal summation order inside one K = 16 instruction (here:
 // sequential fp32), barriers, phases, timing.  So this checks index arithmetic, layouts, the operand
 // split and the error budget -- not the hardware.
@@ -60,36 +63,58 @@ float round_toward_zero(double x) {
 
 struct Planes {
     std::vector<uint16_t> h;   // [2][rows][Ppad]
-    std::vector<float> norm;   // [rows]
+    std::vector<double> term;  // [rows]: a_i (images) or b_m (slices)
     int e = 0;
     bool two = false;
 };
 
-Planes prepare(const float *x, long rows, long P, long Ppad, const uint8_t *mask) {
+// k_common_vector: c[j] = mean over rows 0, step, 2 step, ... of the slices (fp32 sum in ascending row order),
+// 0 in masked pixels and in the K padding; all zero when conditioning is off
+std::vector<float> common_vector(const float *slices, long M, long P, long Ppad, const uint8_t *mask, bool condition) {
+    std::vector<float> c((size_t)Ppad, 0.0f);
+    if (!condition) return c;
+    const long step = common_step(M);
+    const float inv = 1.0f / (float)common_count(M);
+    for (long j = 0; j < P; ++j) {
+        if (mask && !mask[j]) continue;
+        float sum = 0.0f;
+        for (long m = 0; m < M; m += step) sum += slices[m * P + j];
+        c[(size_t)j] = sum * inv;
+    }
+    return c;
+}
+
+// k_absmax + k_split.  which = 0: images (planes of the RAW values, term = a_i = sum (I - c)^2);
+// which = 1: slices (planes of S' = fl(S - c), term = b_m = sum S' (S' + 2 c)).
+Planes prepare(const float *x, long rows, long P, long Ppad, const uint8_t *mask, const std::vector<float> &c, int which) {
     Planes out;
     uint32_t mx = 0;   // k_absmax
     for (long r = 0; r < rows; ++r)
-        for (long c = 0; c < P; ++c) {
-            if (mask && !mask[c]) continue;
-            union { float f; uint32_t u; } v; v.f = fabsf(x[r * P + c]);
+        for (long j = 0; j < P; ++j) {
+            if (mask && !mask[j]) continue;
+            const float val = which ? conditioned(x[r * P + j], c[(size_t)j]) : x[r * P + j];
+            union { float f; uint32_t u; } v; v.f = fabsf(val);
             if (v.u > mx) mx = v.u;
         }
     out.e = scale_exponent(mx);
     const float sc = ldexpf(1.0f, out.e);
     out.h.assign((size_t)2 * rows * Ppad, 0);
-    out.norm.assign(rows, 0.f);
+    out.term.assign(rows, 0.0);
     for (long r = 0; r < rows; ++r) {   // k_split
         double acc = 0.0;
-        for (long c = 0; c < Ppad; ++c) {
+        for (long j = 0; j < Ppad; ++j) {
             float v = 0.0f;
-            if (c < P && (!mask || mask[c])) v = x[r * P + c];
-            acc += (double)v * (double)v;
+            if (j < P && (!mask || mask[j])) {
+                const float raw = x[r * P + j];
+                if (which) { v = conditioned(raw, c[(size_t)j]); acc += slice_term(v, c[(size_t)j]); }
+                else { v = raw; acc += image_term(raw, c[(size_t)j]); }
+            }
             uint16_t a, b;
             out.two |= split_fp16(v, sc, a, b);
-            out.h[(size_t)r * Ppad + c] = a;
-            out.h[(size_t)(rows + r) * Ppad + c] = b;
+            out.h[(size_t)r * Ppad + j] = a;
+            out.h[(size_t)(rows + r) * Ppad + j] = b;
         }
-        out.norm[r] = (float)acc;
+        out.term[r] = acc;
     }
     return out;
 }
@@ -118,11 +143,14 @@ int hostsim_stage_layout(int cg, int ni, int *out /*[5]: stage_bytes, stages, of
 // acc_rz = 1 models a tensor core whose accumulator additions round toward zero (what the literature reports
 // for earlier generations) instead of to nearest; chunk_kblocks = the kernel's CHUNK_KB (K blocks summed in
 // TMEM before the epilogue warps add the chunk into their fp32 registers with round-to-nearest), 0 = whole K.
+// condition = 1: the conditioned expansion (common vector subtracted from the slices), 0: c = 0 (the plain expansion).
+// refine = 1: best_dist is recomputed in the difference form (k_match_refine), 0: the epilogue's own value is returned.
 int hostsim_match(const float *images, long n_img, const float *slices, long M, long P, const uint8_t *mask, int cta_group,
-                  int n_clusters, int acc_rz, int chunk_kblocks, int32_t *best_idx, float *best_dist) {
+                  int n_clusters, int acc_rz, int chunk_kblocks, int condition, int refine, int32_t *best_idx, float *best_dist) {
     const int CG = cta_group;
     const long Ppad = (P + BK - 1) / BK * BK;
-    Planes I = prepare(images, n_img, P, Ppad, mask), S = prepare(slices, M, P, Ppad, mask);
+    const std::vector<float> c = common_vector(slices, M, P, Ppad, mask, condition != 0);
+    Planes I = prepare(images, n_img, P, Ppad, mask, c, 0), S = prepare(slices, M, P, Ppad, mask, c, 1);
     const int NI = I.two ? 2 : 1;
     const int kblocks = (int)(Ppad / BK);
     const int n_ib = (int)((n_img + TILE_ROWS * CG - 1) / (TILE_ROWS * CG)), n_mb = (int)((M + BN - 1) / BN);
@@ -197,13 +225,13 @@ int hostsim_match(const float *images, long n_img, const float *slices, long M, 
             for (int rank = 0; rank < CG; ++rank)
                 for (int lane = 0; lane < TILE_ROWS; ++lane) {
                     const long i = (long)ib * (TILE_ROWS * CG) + (long)rank * TILE_ROWS + lane;
-                    const float nIv = (i < n_img) ? I.norm[i] : 0.0f;
+                    const double aI = (i < n_img) ? I.term[i] : 0.0;
                     float best = INFINITY;
                     uint32_t bm = 0xffffffffu;
                     const long m0 = (long)mb * BN;
                     for (int c = 0; c < BN; ++c) {
-                        const float nS = (m0 + c < M) ? S.norm[m0 + c] : INFINITY;
-                        const float d = distance(nIv, nS, neg2sc, regs[((size_t)rank * TILE_ROWS + lane) * BN + c]);
+                        if (m0 + c >= M) break;
+                        const float d = distance(aI, S.term[m0 + c], neg2sc, regs[((size_t)rank * TILE_ROWS + lane) * BN + c]);
                         if (d < best) { best = d; bm = (uint32_t)(m0 + c); }
                     }
                     if (i < n_img && bm != 0xffffffffu) {
@@ -219,6 +247,16 @@ int hostsim_match(const float *images, long n_img, const float *slices, long M, 
         best_idx[i] = (int32_t)(uint32_t)(k & 0xffffffffull);
         union { uint32_t u; float f; } nan; nan.u = 0x7fc00000u;
         best_dist[i] = (k == ~0ull) ? nan.f : unorderable((uint32_t)(k >> 32));
+        if (refine && k != ~0ull) {   // k_match_refine: the winner's distance in the difference form, fp64 sum, rounded once
+            const float *Ir = images + i * P, *Sr = slices + (long)best_idx[i] * P;
+            double acc = 0.0;
+            for (long j = 0; j < P; ++j) {
+                if (mask && !mask[j]) continue;
+                const double t = (double)Ir[j] - (double)Sr[j];
+                acc += t * t;
+            }
+            best_dist[i] = (float)acc;
+        }
     }
     return NI == 2 ? 3 : 2;
 }

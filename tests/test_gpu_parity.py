@@ -57,19 +57,14 @@ def _rel_l2(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
-def _check_match(bi, bd, images, slices, mask=None, tag="", high_snr=False):
+def _check_match(bi, bd, images, slices, mask=None, tag=""):
     """bi/bd from the GPU; oracle on the same fp32 arrays.  Returns the number of near-ties.
-    high_snr=True is reading s14: where d is a tiny fraction of |I|^2 + |S|^2 (bright, nearly
-    noise-free images) the expanded form cancels in fp32 and the bar is |delta d| <= 1e-6 (|I|^2 + |S|^2);
-    the Poisson configurations never take that branch."""
+    One bar for every matcher and every case (BASELINE.json:north_star): |delta d| <= 1e-4 d, argmin exact unless
+    the oracle's best two distances are within 1e-4 relative.  (The 1e-6 (|I|^2 + |S|^2) form of reading s14 is
+    for the noise-free planted case only, where d = 0; it is asserted there directly.)"""
     oi, od, osd, _ = orc.match(images, slices, mask)
     bi, bd = np.asarray(bi.cpu()), np.asarray(bd.cpu())
     tol_abs = DIST_TOL * np.maximum(od, 1e-30)
-    if high_snr:
-        keep = slice(None) if mask is None else np.flatnonzero(mask)
-        nI = (np.asarray(images)[:, keep].astype(np.float64) ** 2).sum(1)
-        nS = (np.asarray(slices)[oi][:, keep].astype(np.float64) ** 2).sum(1)
-        tol_abs = np.maximum(tol_abs, 1e-6 * (nI + nS))
     assert np.all(np.abs(bd - od) <= tol_abs + 1e-6 * (od == 0)), "%s distances differ: max rel %.3e" % (
         tag, float(np.max(np.abs(bd - od) / np.maximum(od, 1e-30))))
     near = (osd - od) <= tol_abs
@@ -279,8 +274,9 @@ def match_planted_ties_and_general_values(spf, variant):
     # large counts (> 2048: not exact in one fp16 term) and a wide dynamic range
     I2 = rng.poisson(3000.0 * S[rng.integers(0, M, 9)]).astype(np.float32)
     bi, bd = ctx.spf_match(_dev(I2), _dev((3000.0 * S).astype(np.float32)))
-    # d ~ 3e-4 (|I|^2 + |S|^2) here: the cancellation-limited case of reading s14 for the expanded-form kernels
-    _check_match(bi, bd, I2, (3000.0 * S).astype(np.float32), None, "large counts", high_snr=True)
+    # d ~ 3e-4 (|I|^2 + |S|^2) here: the plain expansion would cancel in fp32; the tensor-core matcher conditions
+    # the expansion and recomputes the winner's distance in the difference form, so the bar is the same 1e-4 d
+    _check_match(bi, bd, I2, (3000.0 * S).astype(np.float32), None, "large counts")
     # scaling: d(aI, aS) = a^2 d with a a power of two is exact through the rescale
     bi4, bd4 = ctx.spf_match(_dev(4 * I2), _dev((4 * (3000.0 * S).astype(np.float32))))
     assert np.array_equal(bi4.cpu().numpy(), bi.cpu().numpy())
@@ -289,7 +285,7 @@ def match_planted_ties_and_general_values(spf, variant):
     perm = rng.permutation(M)
     S3p = (3000.0 * S[perm]).astype(np.float32)
     bip, bdp = ctx.spf_match(_dev(I2), _dev(S3p))
-    _check_match(bip, bdp, I2, S3p, None, "permuted", high_snr=True)
+    _check_match(bip, bdp, I2, S3p, None, "permuted")
     assert np.allclose(bdp.cpu().numpy(), bd.cpu().numpy(), rtol=1e-5)
     # empty image set is a no-op; M = 0 with images is an error
     assert ctx.spf_match(_dev(I[:0]), _dev(S))[0].shape == (0,)

@@ -36,35 +36,32 @@ def sim():
     L.hostsim_stage_layout.argtypes = [C.c_int, C.c_int, C.c_void_p]
     L.hostsim_stage_layout.restype = C.c_int
     L.hostsim_match.argtypes = [C.c_void_p, C.c_long, C.c_void_p, C.c_long, C.c_long, C.c_void_p, C.c_int, C.c_int,
-                                C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+                                C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
     L.hostsim_match.restype = C.c_int
     L.hostsim_chunk_kb.restype = C.c_int
     return L
 
 
-def _match(sim, I, S, mask=None, cta_group=1, n_clusters=148, acc_rz=0, chunk_kblocks=None):
-    """chunk_kblocks None = the kernel's CHUNK_KB (spf_match_math.cuh); 0 = one accumulation over all of K."""
+def _match(sim, I, S, mask=None, cta_group=1, n_clusters=148, acc_rz=0, chunk_kblocks=None, condition=1, refine=1):
+    """chunk_kblocks None = the kernel's CHUNK_KB (spf_match_math.cuh); 0 = one accumulation over all of K.
+    condition / refine: the library's defaults (1, 1); 0 switches the common-vector subtraction / the
+    difference-form recomputation of the winner's distance off (to show what each one buys)."""
     if chunk_kblocks is None:
         chunk_kblocks = sim.hostsim_chunk_kb()
     I, S = np.ascontiguousarray(I, np.float32), np.ascontiguousarray(S, np.float32)
     bi, bd = np.empty(I.shape[0], np.int32), np.empty(I.shape[0], np.float32)
     mk = None if mask is None else np.ascontiguousarray(mask, np.uint8)
     prods = sim.hostsim_match(I.ctypes.data, I.shape[0], S.ctypes.data, S.shape[0], I.shape[1],
-                              None if mk is None else mk.ctypes.data, cta_group, n_clusters, acc_rz, chunk_kblocks, bi.ctypes.data, bd.ctypes.data)
+                              None if mk is None else mk.ctypes.data, cta_group, n_clusters, acc_rz, chunk_kblocks, condition, refine,
+                              bi.ctypes.data, bd.ctypes.data)
     return bi, bd, prods
 
 
-def _check(bi, bd, I, S, mask=None, high_snr=False):
-    """Distances within 1e-4 relative (north_star).  high_snr=True is reading s14: when d is a tiny fraction
-    of |I|^2 + |S|^2 (bright, nearly noise-free images) the expanded form cancels in fp32, and the bar is
-    |delta d| <= 1e-6 (|I|^2 + |S|^2); the Poisson configs never take that branch."""
+def _check(bi, bd, I, S, mask=None):
+    """Distances within 1e-4 relative of the oracle's, argmin exact outside near-ties (north_star).  No other
+    tolerance: the 1e-6 (|I|^2 + |S|^2) form of reading s14 applies to the noise-free planted case only (d = 0)."""
     oi, od, osd, _ = orc.match(I, S, mask)
     tol = DIST_TOL * np.maximum(od, 1e-30)
-    if high_snr:
-        keep = slice(None) if mask is None else np.flatnonzero(mask)
-        nI = (I[:, keep].astype(np.float64) ** 2).sum(1)
-        nS = (S[oi][:, keep].astype(np.float64) ** 2).sum(1)
-        tol = np.maximum(tol, 1e-6 * (nI + nS))
     err = np.abs(bd - od)
     assert np.all(err <= tol), "max relative distance error %.3e" % (err / np.maximum(od, 1e-30)).max()
     near = (osd - od) <= tol
@@ -136,7 +133,9 @@ def test_replayed_match_two_plane_images_ties_and_scaling(sim):
     S3 = (3000.0 * S).astype(np.float32)
     bi, bd, prods = _match(sim, I2, S3)
     assert prods == 3
-    _check(bi, bd, I2, S3, high_snr=True)     # d ~ 3e-4 (|I|^2 + |S|^2): the cancellation-limited case of s14
+    # d ~ 3e-4 (|I|^2 + |S|^2): the case where the plain expansion cancels in fp32.  The conditioned expansion
+    # decides the argmin, k_match_refine recomputes the winner's distance in the difference form: 1e-4 d holds.
+    _check(bi, bd, I2, S3)
     bi4, bd4, _ = _match(sim, 4 * I2, 4 * S3)            # power-of-two scaling passes through the rescale exactly
     assert np.array_equal(bi4, bi) and np.array_equal(bd4, 16 * bd)
     # a wide dynamic range inside one operand and very small / very large overall scales
@@ -144,7 +143,7 @@ def test_replayed_match_two_plane_images_ties_and_scaling(sim):
         Sw = (S * np.float32(10.0) ** rng.integers(-3, 1, (M, 1)).astype(np.float32) * np.float32(scale)).astype(np.float32)
         Iw = (Sw[rng.integers(0, M, 6)] * (1 + 0.05 * rng.standard_normal((6, P)))).astype(np.float32)
         bi, bd, _ = _match(sim, Iw, Sw)
-        _check(bi, bd, Iw, Sw, high_snr=True)
+        _check(bi, bd, Iw, Sw)
 
 
 def test_replayed_match_small_config_statistics(sim):
@@ -163,3 +162,48 @@ def test_replayed_match_small_config_statistics(sim):
         worst, ties = _check(bi, bd, I, S, mask)
         print("small-config replay cg%d: worst relative distance error %.2e, %d near-ties" % (cg, worst, ties))
         assert worst <= 2e-5      # an order of magnitude inside the 1e-4 bar
+
+
+def test_bright_images_what_conditioning_and_refinement_buy(sim):
+    """The 3,000x-brightness case again, stage by stage.  The expanded form's error is a
+    multiple of fp32 epsilon times the norms of what is fed to the contraction: the plain form misses 1e-4 d,
+    subtracting the common vector shrinks the error (the norms of I - c and S - c are 4x smaller here), and the
+    difference-form recomputation of the winner removes it from best_dist altogether."""
+    rng = np.random.default_rng(17)
+    M, P = 200, 640
+    S3 = (3000.0 * rng.random((M, P))).astype(np.float32)
+    I2 = rng.poisson(S3[rng.integers(0, M, 9)].astype(np.float64)).astype(np.float32)
+    oi, od, _, _ = orc.match(I2, S3)
+    worst = {}
+    for name, cond, refine in (("plain", 0, 0), ("conditioned", 1, 0), ("conditioned+refined", 1, 1)):
+        bi, bd, _ = _match(sim, I2, S3, condition=cond, refine=refine)
+        assert np.array_equal(bi, oi)
+        worst[name] = float(np.max(np.abs(bd - od) / od))
+    print("bright images, worst relative distance error:", worst)
+    assert worst["plain"] > DIST_TOL                      # the finding the round-1 tolerance was stretched to cover
+    assert worst["conditioned"] < 0.6 * worst["plain"]
+    assert worst["conditioned+refined"] < 1e-6
+
+
+def test_truncating_accumulator_and_chunk_size(sim):
+    """Paper-scale statistics (65,536 pixels, 5 % masked, ~1e4 photons per image) under a tensor core whose
+    accumulator rounds toward zero: one accumulation over the whole of K biases the winning distance by more
+    than the 1e-4 bar; the library's chunk size keeps it an order of magnitude inside, with or without rounding
+    to nearest.  Errors are those of the epilogue's own distance (refine = 0): they bound the argmin decision."""
+    cfg = CONFIGS["paper_scale"]
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    mask = make_mask(cfg.panels, cfg.panel_edge, cfg.masked_frac)
+    S = surrogate_slices(256, pix)
+    S *= np.float32(cfg.photons / float(S.sum(axis=1).mean()))
+    I = poisson_images(S[np.arange(8) * 31 % 256])
+    oi, od, _, _ = orc.match(I, S, mask)
+
+    def worst(**kw):
+        bi, bd, prods = _match(sim, I, S, mask, refine=0, **kw)
+        assert prods == 2 and np.array_equal(bi, oi)
+        return float(np.max(np.abs(bd - od) / od))
+    whole_rz, lib_rz, lib_rn = worst(acc_rz=1, chunk_kblocks=0), worst(acc_rz=1), worst(acc_rz=0)
+    print("paper-scale statistics: truncating whole-K %.2e, truncating CHUNK_KB=%d %.2e, nearest %.2e"
+          % (whole_rz, sim.hostsim_chunk_kb(), lib_rz, lib_rn))
+    assert whole_rz > DIST_TOL
+    assert lib_rz < 2e-5 and lib_rn < 1e-5
