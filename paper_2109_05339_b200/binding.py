@@ -11,7 +11,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libspf.so")
+# SPF_DEBUG=1 loads the build with device-side asserts (python -m paper_2109_05339_b200.build under the same variable)
+LIB_PATH = os.path.join(_HERE, "libspf_debug.so" if os.environ.get("SPF_DEBUG", "0") == "1" else "libspf.so")
 
 SPF_OUT_COMPLEX = 0
 SPF_OUT_INTENSITY = 1

@@ -13,6 +13,14 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "--expt-relaxed-constexpr"]
 
 
+if os.environ.get("SPF_DEBUG", "0") == "1":
+    # device-side asserts on the invariants the TMA / tcgen05 kernels rely on; objects of a
+    # debug build are kept apart so that switching the flag never links a mix
+    NVCC_FLAGS += ["-DSPF_DEBUG"]
+    LIB = os.path.join(_HERE, "libspf_debug.so")
+_OBJ_SUFFIX = ".debug.o" if "-DSPF_DEBUG" in NVCC_FLAGS else ".o"
+
+
 def _newest(paths):
     return max(os.path.getmtime(p) for p in paths)
 
@@ -24,7 +32,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
     objs, procs = [], []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
-        o = os.path.join(CSRC, src.replace(".cu", ".o"))
+        o = os.path.join(CSRC, src.replace(".cu", _OBJ_SUFFIX))
         objs.append(o)
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_time):
             cmd = [nvcc, *NVCC_FLAGS, "-c", s, "-o", o] + (["-Xptxas", "-v"] if verbose else [])

@@ -14,6 +14,7 @@
 // Coordinates (rotation, scaling to cells, split into integer cell + fraction) are fp64: an fp32
 // error of one ulp at |xi| ~ 150 cells is 1.5e-5 cells, which a model that fills the grid turns
 // into a 1e-5 relative error, the whole parity budget.
+#include <assert.h>
 #include <limits.h>
 #include <math.h>
 
@@ -180,6 +181,17 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, a.cap_bytes, COOP);
         bz = g.bz; S1 = g.S1;
         staged = g.ok;
+#ifdef SPF_DEBUG
+        // invariants of the bulk tensor copies: 128-byte aligned destinations, the box
+        // inside the tile capacity, a box size that is on the tensor-map menu, transaction bytes below 2^20
+        if (staged && tid == 0) {
+            assert((ptx::smem_u32(s_tile) & 127u) == 0u && ((uint32_t)(S1 * CELL) & 127u) == 0u);
+            assert((uint32_t)(Lx * S1 * CELL) <= a.cap_bytes && (uint32_t)(Lx * g.by * bz * CELL) < (1u << 20));
+            assert(g.by >= SPF_BOX_MIN && g.by <= SPF_BOX_MAX && bz >= SPF_BOX_MIN && bz <= SPF_BOX_MAX);
+            assert(g.by % SPF_BOX_STEP == 0 && bz % SPF_BOX_STEP == 0 && g.by * bz <= S1);
+            assert(lox >= 0 && loy >= 0 && loz >= 0 && lox + Lx <= a.np && loy + Ly <= a.np && loz + Lz <= a.sz);
+        }
+#endif
         if (staged && tid < 32) {
             const uint32_t bar = ptx::smem_u32(&s_bar);
             if (tid == 0) ptx::mbar_expect_tx(bar, (uint32_t)(Lx * g.by * bz * CELL));
