@@ -231,7 +231,7 @@ def run_spf(args, cfg):
     # device self-check passes in a child process (paper_2109_05339_b200/selfcheck.py).  Opt-in until those kernels
     # have been cleared on hardware: the default run never launches an unverified kernel.
     variants = (ctx.spf_autotune() if args.native else
-                {"slice_staged": False, "slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False,
+                {"slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False,
                  "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
     info = ctx.info
     d_model = torch.from_numpy(model).to(dev)
@@ -330,7 +330,7 @@ def run_spf(args, cfg):
             "config": {"workload": cfg.name, "N": cfg.N, "n_fine": info.n_fine, "w": info.w, "P": cfg.P, "M": cfg.M,
                        "n_img_per_gpu": cfg.n_img, "eps": cfg.eps, "masked_frac": cfg.masked_frac,
                        "grid_is_real": bool(info.grid_is_real),
-                       "kernel_variants": {"slice": {0: "tma_staged, thread per point", 1: "global_gather, thread per point",
+                       "kernel_variants": {"slice": {1: "global_gather, thread per point",
                                                      2: "tma_staged, warp per point", 3: "global_gather, warp per point"}[variants["slice_impl"]],
                                            "match": ("tcgen05 cta_group::%d" % variants["match_cta_group"]) if variants["match_impl"] == 0
                                                     else "cuda_core difference form (library default; tcgen05 variant %s)" % ("failed its self-check" if args.native else "not requested"),

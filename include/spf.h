@@ -185,10 +185,10 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
 
 /*
  * Kernel variants and test/benchmark knobs (defaults in brackets):
- *   "slice_impl":  [1] = plain global-memory gather, one thread per point;
- *                  0 = tile staged in shared memory by TMA, one thread per point gathers from it;
- *                  2 = the same tile, a warp per point: 32 lanes read an 8 x 8 window per x-plane with no
- *                      bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; w = 10 runs as 0);
+ *   "slice_impl":  [1] = plain global-memory gather, one thread per point (the reference form);
+ *                  2 = a warp per point, tile staged in shared memory by TMA: 32 lanes read an 8 x 8 window per x-plane
+ *                      with no bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; blocks whose box
+ *                      does not fit the tile, and every block at w = 10, run as 3);
  *                  3 = the warp-per-point gather straight from global memory (no TMA, mbarrier or tile;
  *                      8 x 8 window at w = 7, 16-cell window at w = 10)
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model

@@ -154,8 +154,8 @@ class SpfContext:
     def spf_autotune(self, timeout_s: float = 240.0) -> dict:
         """Switch on the faster kernel variants that pass the device self-check (selfcheck.py, run once per
         process in a child process so that a faulting variant cannot take this process's CUDA context with
-        it): for slicing the verified variant that the check timed fastest (TMA-staged, one thread or one
-        warp per point), for matching the tcgen05 GEMM (cta_group::2 when verified, else single CTA),
+        it): for slicing the verified variant that the check timed fastest (one warp per point, TMA-staged
+        or straight from global memory), for matching the tcgen05 GEMM (cta_group::2 when verified, else single CTA),
         else the CUDA-core matcher stays.  Returns {variant: bool} plus "slice_impl" / "match_impl" /
         "match_cta_group" = the options now in force."""
         from .selfcheck import verified_variants, fastest_slice_impl

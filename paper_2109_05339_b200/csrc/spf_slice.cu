@@ -52,18 +52,21 @@ __device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t
 }
 
 // Kernel variants (option "slice_impl"):
-//   IMPL_GLOBAL  1  one thread per point, w^3 loads straight from the grid in global memory (L1/L2)
-//   IMPL_STAGED  0  tile staged by TMA, one thread per point gathers from shared memory
+//   IMPL_GLOBAL  1  one thread per point, w^3 loads straight from the grid in global memory (L1/L2): the
+//                   reference gather (the definition written out), and the library's starting variant
 //   IMPL_COOP    2  tile staged by TMA, a WARP gathers each point: lane (h, k) reads rows h, h + 4 and
 //                   cell k of the point's 8 x 8 window in every x-plane -- 32 consecutive-bank words per
 //                   load, no bank conflicts (spf_slice_math.cuh) -- and a shuffle tree adds the 32
-//                   partial sums.  One thread per point has its lanes scattered over the tile (the
-//                   rotated lattice is generic), which costs a conflict degree of ~3.5 per load
-//                   (DESIGN.md section 5); the warp-per-point form needs 14 conflict-free loads + 4
-//                   weight loads per point instead of 343 loads / 32 lanes x 3.5.
+//                   partial sums: 14 conflict-free loads + 4 weight loads per point.  Blocks whose box does
+//                   not fit the tile, and every block at w > 8, walk the grid in global memory instead
+//                   (the IMPL_GCOOP path below).
 //   IMPL_GCOOP   3  the same warp-per-point walk straight from the grid in global memory: no TMA, no
 //                   mbarrier, no tile -- each load is four 32-byte row segments instead of 32 scattered words
-enum { IMPL_STAGED = 0, IMPL_GLOBAL = 1, IMPL_COOP = 2, IMPL_GCOOP = 3 };
+// (A TMA-staged one-thread-per-point form existed in round 1 as variant 0.  With one thread per point the 32 lanes
+// of a warp are scattered over the tile and every load replays ~3.8 times on bank conflicts -- 41 wavefronts per
+// point against 18 here, tests/test_hostsim_slice_math.py::test_bank_conflicts... -- so it could not reach half of
+// the shared-memory roofline by construction and was deleted.)
+enum { IMPL_GLOBAL = 1, IMPL_COOP = 2, IMPL_GCOOP = 3 };
 #define SPF_COOP_WTS_BYTES (SPF_PATCH * SPF_COOP_STRIDE * 4)   // 14,336 = 112 x 128
 
 // The cooperative gather of one warp over its 32 points (variants 2 and 3).  `tile` is the staged box in
@@ -118,7 +121,7 @@ __device__ __forceinline__ void coop_sweep(const float *tile, IDX cell, int S1, 
 // W = 0: runtime kernel width (any w <= SPF_MAX_W), else compile-time.
 template <int W, bool REAL, int OUTK, int IMPL>
 __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMPL_GCOOP) ? 4 : 3) k_slice(const __grid_constant__ SliceArgs a) {
-    constexpr bool STAGED = (IMPL == IMPL_STAGED || IMPL == IMPL_COOP);
+    constexpr bool STAGED = (IMPL == IMPL_COOP);
     constexpr bool COOP = (IMPL == IMPL_COOP);
     constexpr bool GCOOP = (IMPL == IMPL_GCOOP);
     constexpr bool WIDE = GCOOP && W > 8;      // 16-cell window, global memory only (spf_slice_math.cuh)
@@ -178,7 +181,7 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         // a patch with no pixel at all (cannot happen with the tables build_patches makes) has lo > hi: not staged
         const bool any = s_hi[0] >= lox;
         const int Lx = any ? s_hi[0] - lox + w : 0, Ly = any ? s_hi[1] - loy + w : 0, Lz = any ? s_hi[2] - loz + w : 0;
-        const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, a.cap_bytes, COOP);
+        const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, a.cap_bytes);
         bz = g.bz; S1 = g.S1;
         staged = g.ok;
 #ifdef SPF_DEBUG
@@ -245,16 +248,11 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         }
         const float *tile = reinterpret_cast<const float *>(s_tile);
         const int cell = active ? (px - lox) * S1 + (py - loy) * bz + (pz - loz) : -1;
-        if (COOP) {
-            // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates
-            if (bz == 24) coop_sweep<REAL, 24, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
-            else if (bz == 8) coop_sweep<REAL, 8, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
-            else coop_sweep<REAL, 40, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
-            if (!active) return;
-        } else {
-            if (!active) return;
-            c = spfm::gather<WMAX, REAL>(tile + (size_t)cell * E, S1, bz, w, wx, wy, wz);
-        }
+        // bz is 8, 24 or 40 (tile_geom): one loop per value, so the row offsets are immediates
+        if (bz == 24) coop_sweep<REAL, 24, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
+        else if (bz == 8) coop_sweep<REAL, 8, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
+        else coop_sweep<REAL, 40, int>(tile, cell, S1, bz, w, wts_warp, lane, c);
+        if (!active) return;
     } else if (COOP || GCOOP) {
         // the same warp-per-point walk straight from the padded grid (L1/L2): variant 3, and the blocks of
         // variant 2 whose box does not fit the tile.  The 8 x 8 window reads one row and one cell past the
@@ -300,11 +298,9 @@ int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
     uint32_t smem = 0;
     args.cap_bytes = 0;
     if (IMPL == IMPL_GCOOP) smem = W > 8 ? (uint32_t)(SPF_PATCH * SPF_COOPW_STRIDE * 4) : (uint32_t)SPF_COOP_WTS_BYTES;   // the parked weights only
-    if (IMPL == IMPL_STAGED || IMPL == IMPL_COOP) {
-        // w = 10: an 8 x 16 patch needs up to 73 KB on the real grid (seeded replay of the Slicing-heavy geometry),
-        // 72 KB stages all but a fraction of a percent of the blocks and still leaves three blocks per SM
-        args.cap_bytes = W == 10 ? 72u * 1024u : (IMPL == IMPL_COOP ? 48u : 36u) * 1024u * (REAL ? 1u : 2u);
-        smem = args.cap_bytes + (IMPL == IMPL_COOP ? (uint32_t)SPF_COOP_WTS_BYTES : 0u);
+    if (IMPL == IMPL_COOP) {
+        args.cap_bytes = 48u * 1024u * (REAL ? 1u : 2u);
+        smem = args.cap_bytes + (uint32_t)SPF_COOP_WTS_BYTES;
         SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         // three (real grid) or two (complex grid) blocks per SM only fit with the largest shared-memory carve-out
         SPF_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
@@ -326,11 +322,9 @@ int launch_slice_w(spf_ctx *ctx, SliceArgs &args, int impl, cudaStream_t st) {
         case 7:
             if (impl == IMPL_COOP) return launch_slice<7, REAL, OUTK, IMPL_COOP>(ctx, args, st);
             if (impl == IMPL_GCOOP) return launch_slice<7, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
-            if (impl == IMPL_STAGED) return launch_slice<7, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
             return launch_slice<7, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
-        case 10:   // 10 x 10 window: the cooperative form (8 x 8) does not apply
-            if (impl == IMPL_STAGED || impl == IMPL_COOP) return launch_slice<10, REAL, OUTK, IMPL_STAGED>(ctx, args, st);
-            if (impl == IMPL_GCOOP) return launch_slice<10, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
+        case 10:   // 10 x 10 window: the staged 8 x 8 form does not apply, variants 2 and 3 both walk global memory (16-cell window)
+            if (impl == IMPL_COOP || impl == IMPL_GCOOP) return launch_slice<10, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
             return launch_slice<10, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         default: return launch_slice<0, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);  // any other width: runtime-w global gather
     }
@@ -366,7 +360,7 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.maps = real ? ctx->maps_r : ctx->maps_c;
     args.fault = ctx->d_fault; args.abort_flag = ctx->d_abort;
     const int impl = ctx->opt_slice_impl;
-    if ((impl == IMPL_STAGED || impl == IMPL_COOP) && !ctx->maps_ok)
+    if (impl == IMPL_COOP && ctx->w <= 8 && !ctx->maps_ok)
         return spf_set_err(ctx, SPF_ECUDA, "spf_slice: slice_impl %d needs the TMA tensor maps, which could not be encoded: %s", impl,
                            ctx->maps_err.c_str());
     if (real) {

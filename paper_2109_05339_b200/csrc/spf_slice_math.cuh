@@ -158,30 +158,25 @@ SPF_HD c2 gather(const float *base, int sx, int sy, int w, const float (&wx)[WMA
 }
 
 // ------------------------------------------------------------------------------------------
-// shared-memory tile of the staged kernels (k_slice, slice_impl 0 and 2) and the cooperative gather
+// shared-memory tile of the staged kernel (k_slice, slice_impl 2) and the cooperative gather
 // ------------------------------------------------------------------------------------------
 // A block's points touch the box [lo, hi + w) of padded cells; L = hi - lo + w per axis.  The box is
 // staged one x-plane per TMA copy with a (by x bz)-cell box taken from a fixed menu (one tensor map
 // per size), rows written densely (row pitch = bz cells), planes S1 cells apart (128-byte aligned).
-//   per-lane gather (coop = false): by, bz = L rounded up to the menu step.
-//   cooperative gather (coop = true, w <= 8): a warp's lanes read rows t2 = h, h + 4 (h = lane >> 3)
-//     and cells t3 = lane & 7 of every x-plane, i.e. an 8 x 8 window per point, so the box needs
-//     8 - w spare rows and cells; bz is 8, 24 or 40 (bz = 8 mod 16), which puts the four rows a warp
-//     reads at once (offsets 0, bz, 2 bz, 3 bz) into four disjoint groups of 8 banks: no conflicts.
+// A warp's lanes read rows t2 = h, h + 4 (h = lane >> 3) and cells t3 = lane & 7 of every x-plane, i.e.
+// an 8 x 8 window per point (w <= 8), so the box needs 8 - w spare rows and cells; bz is 8, 24 or 40
+// (bz = 8 mod 16), which puts the four rows a warp reads at once (offsets 0, bz, 2 bz, 3 bz) into four
+// disjoint groups of 8 banks: no conflicts.
 struct TileGeom { int by, bz, S1; bool ok; };
-SPF_HD TileGeom tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, uint32_t cap_bytes, bool coop) {
+SPF_HD TileGeom tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, uint32_t cap_bytes) {
     TileGeom g;
-    const int ey = coop ? Ly + 8 - w : Ly, ez = coop ? Lz + 8 - w : Lz;
+    const int ey = Ly + 8 - w, ez = Lz + 8 - w;
     g.by = (ey + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP;
     if (g.by < SPF_BOX_MIN) g.by = SPF_BOX_MIN;
-    if (coop) g.bz = ez <= 8 ? 8 : (ez <= 24 ? 24 : 40);
-    else {
-        g.bz = (ez + SPF_BOX_STEP - 1) / SPF_BOX_STEP * SPF_BOX_STEP;
-        if (g.bz < SPF_BOX_MIN) g.bz = SPF_BOX_MIN;
-    }
+    g.bz = ez <= 8 ? 8 : (ez <= 24 ? 24 : 40);
     const int per128 = 128 / cell_bytes;
     g.S1 = (g.by * g.bz + per128 - 1) / per128 * per128;
-    g.ok = Lx > 0 && g.by <= SPF_BOX_MAX && g.bz <= SPF_BOX_MAX && ez <= SPF_BOX_MAX &&
+    g.ok = w <= 8 && Lx > 0 && g.by <= SPF_BOX_MAX && g.bz <= SPF_BOX_MAX && ez <= SPF_BOX_MAX &&
            (uint64_t)Lx * (uint64_t)g.S1 * (uint64_t)cell_bytes <= (uint64_t)cap_bytes;
     return g;
 }

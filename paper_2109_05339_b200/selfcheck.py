@@ -2,7 +2,7 @@
 
 libspf has several implementations of each hot kernel: one with the least machinery (plain global
 gather; CUDA-core difference-form matcher) and faster ones (warp-per-point gather from global memory;
-TMA-staged shared-memory gather, one thread or one warp per point; tcgen05 GEMM on single CTAs or cta_group::2 pairs).  The library starts on the first;
+TMA-staged shared-memory gather, one warp per point; tcgen05 GEMM on single CTAs or cta_group::2 pairs).  The library starts on the first;
 `SpfContext.spf_autotune()` switches on the faster ones that pass this self-check on the device at
 hand, and among the slicing variants that pass, the one the check timed fastest.
 
@@ -33,8 +33,8 @@ import sys
 import time
 
 # least machinery first: classic CUDA (no TMA / mbarrier / tcgen05), then TMA + mbarrier, then tcgen05, CTA pairs last
-VARIANTS = ("slice_gcoop", "slice_staged", "slice_coop", "match_cg1", "match_cg2")
-SLICE_IMPL = {"slice_staged": 0, "slice_coop": 2, "slice_gcoop": 3}
+VARIANTS = ("slice_gcoop", "slice_coop", "match_cg1", "match_cg2")
+SLICE_IMPL = {"slice_coop": 2, "slice_gcoop": 3}
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
 

@@ -62,10 +62,10 @@ void hostsim_slice(const float *grid, int is_real, int np, int sz, int nf, int h
     }
 }
 
-// Replay of one k_slice<STAGED | COOP> launch on the CPU, block by block (spf_slice.cu): patch table ->
+// Replay of one k_slice<COOP | GCOOP> launch on the CPU, block by block (spf_slice.cu): patch table ->
 // per-point cell + fraction -> block bounding box -> tile_geom -> the tile image TMA would write (one
-// (by x bz) box per x-plane at pitch S1, zeros outside the padded grid) -> gather from the tile, either
-// one thread per point (coop = 0) or lane by lane as a warp does it (coop = 1; coop = 2 is variant 3, the same
+// (by x bz) box per x-plane at pitch S1, zeros outside the padded grid) -> gather from the tile, lane by
+// lane as a warp does it (coop = 1; coop = 2 is variant 3, the same
 // walk with no tile, straight from the grid: weights parked in the
 // 28-float layout, groups of 8 points, partial sums added by the multi-value butterfly).  Everything the tile image
 // does NOT receive from a copy is NaN, so a read outside the staged box poisons the result even
@@ -109,8 +109,8 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
         }
         const bool any = hi[0] >= lo[0];
         const int Lx = any ? hi[0] - lo[0] + w : 0, Ly = any ? hi[1] - lo[1] + w : 0, Lz = any ? hi[2] - lo[2] + w : 0;
-        spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, cap_bytes, coop != 0);
-        if (coop == 2 || (coop && w > 8)) g.ok = false;        // variant 3: no tile at all (and no staged cooperative form beyond w = 8)
+        spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, CELL, cap_bytes);
+        if (coop == 2) g.ok = false;        // variant 3: no tile at all (tile_geom itself refuses w > 8)
         std::vector<float> tile;
         if (g.ok) {
             n_staged++;
@@ -127,7 +127,7 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
             n_global++;
         }
         spfm::c2 res[PATCH];
-        if (coop) {
+        {
             // weights parked in the 28-float layout (slots of empty lanes hold NaN: they must never be read)
             const bool wide = w > 8;                 // variant 3 at w = 10: 16-cell window, 44-float weight sets
             const int wstride = wide ? SPF_COOPW_STRIDE : SPF_COOP_STRIDE;
@@ -197,19 +197,6 @@ void hostsim_slice_blocks(const float *grid, int is_real, int np, int sz, int nf
                         res[t].x = pr[spfm::mr8_result_lane(u)][0]; res[t].y = pi[spfm::mr8_result_lane(u)][0];
                     }
                 }
-        } else {
-            for (int t = 0; t < PATCH; ++t) {
-                if (jj[t] < 0) continue;
-                if (g.ok) {
-                    const float *base = tile.data() + (size_t)((px[t] - lo[0]) * g.S1 + (py[t] - lo[1]) * g.bz + (pz[t] - lo[2])) * E;
-                    res[t] = is_real ? spfm::gather<SPF_MAX_W, true>(base, g.S1, g.bz, w, wx[t], wy[t], wz[t])
-                                     : spfm::gather<SPF_MAX_W, false>(base, g.S1, g.bz, w, wx[t], wy[t], wz[t]);
-                } else {
-                    const float *base = grid + ((size_t)((size_t)px[t] * np + py[t]) * sz + pz[t]) * E;
-                    res[t] = is_real ? spfm::gather<SPF_MAX_W, true>(base, np * sz, sz, w, wx[t], wy[t], wz[t])
-                                     : spfm::gather<SPF_MAX_W, false>(base, np * sz, sz, w, wx[t], wy[t], wz[t]);
-                }
-            }
         }
         for (int t = 0; t < PATCH; ++t)
             if (jj[t] >= 0) { out[2 * (m * P + jj[t])] = res[t].x; out[2 * (m * P + jj[t]) + 1] = res[t].y; }
@@ -265,8 +252,8 @@ long hostsim_count_uneven(const float *A, int N) {
 }
 
 // tile geometry alone, for the menu / capacity tests
-void hostsim_tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, unsigned cap, int coop, int *out4) {
-    const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, cell_bytes, cap, coop != 0);
+void hostsim_tile_geom(int Lx, int Ly, int Lz, int w, int cell_bytes, unsigned cap, int *out4) {
+    const spfm::TileGeom g = spfm::tile_geom(Lx, Ly, Lz, w, cell_bytes, cap);
     out4[0] = g.by; out4[1] = g.bz; out4[2] = g.S1; out4[3] = g.ok ? 1 : 0;
 }
 

@@ -131,8 +131,8 @@ def test_autotune_picks_the_fastest_verified_slicing_variant():
     from paper_2109_05339_b200.selfcheck import fastest_slice_impl
     ok = lambda ms, g=10.0: {"ok": True, "metrics": {"slice_ms": ms, "slice_ms_global": g}}
     assert fastest_slice_impl({}) == 1
-    assert fastest_slice_impl({"slice_staged": ok(5.0), "slice_coop": ok(3.0)}) == 2
-    assert fastest_slice_impl({"slice_staged": ok(2.0), "slice_coop": ok(3.0)}) == 0
-    assert fastest_slice_impl({"slice_staged": ok(12.0), "slice_coop": {"ok": False, "metrics": {"slice_ms": 1.0}}}) == 1
+    assert fastest_slice_impl({"slice_gcoop": ok(5.0), "slice_coop": ok(3.0)}) == 2
+    assert fastest_slice_impl({"slice_gcoop": ok(2.0), "slice_coop": ok(3.0)}) == 3
+    assert fastest_slice_impl({"slice_gcoop": ok(12.0), "slice_coop": {"ok": False, "metrics": {"slice_ms": 1.0}}}) == 1
     assert fastest_slice_impl({"slice_coop": {"ok": True, "metrics": {}}}) == 1
-    assert fastest_slice_impl({"slice_gcoop": ok(4.0), "slice_coop": ok(6.0), "slice_staged": {"ok": False, "metrics": {}}}) == 3
+    assert fastest_slice_impl({"slice_gcoop": ok(4.0), "slice_coop": ok(6.0)}) == 3

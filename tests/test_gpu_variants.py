@@ -1,7 +1,7 @@
 """GPU parity of the faster kernel variants (-m gpu; collected after tests/test_gpu_parity.py).
 
-`slice_impl = 3` (warp-per-point gather from global memory), `0` / `2` (TMA-staged shared-memory gather, one
-thread / one warp per point) and
+`slice_impl = 3` (warp-per-point gather from global memory), `2` (the same gather from a TMA-staged
+shared-memory tile) and
 `match_impl = 0` (the tcgen05 GEMM, on single CTAs and on `cta_group::2` pairs) are held to the same bars as the default variants: slices relative L2 <= 1e-5 against the oracle,
 distances <= 1e-4, argmin exact outside near-ties.  Before a variant is launched in this process its
 device self-check (paper_2109_05339_b200/selfcheck.py) must have passed in a child process; if it did
@@ -44,14 +44,14 @@ def _require(verified, variant):
         pytest.fail("device self-check of %s did not pass (status %s): %s" % (variant, r["status"], r["detail"]))
 
 
-@pytest.mark.parametrize("variant", ["match_cg1", "slice_gcoop", "slice_staged", "slice_coop", "match_cg2"])
+@pytest.mark.parametrize("variant", ["slice_gcoop", "slice_coop", "match_cg1", "match_cg2"])
 def test_variant_selfcheck(verified, variant):
     _require(verified, variant)
 
 
 # --------------------------------------------------------------------------------- staged slicing
 
-STAGED = [("slice_gcoop", 3), ("slice_staged", 0), ("slice_coop", 2)]
+STAGED = [("slice_gcoop", 3), ("slice_coop", 2)]
 
 
 @pytest.mark.parametrize("variant,impl", STAGED)
@@ -62,14 +62,14 @@ def test_staged_slice_tiny_full(spf, tiny, verified, force_complex, layout, vari
 
 
 def test_staged_slice_equals_the_layout_free_result(spf, tiny, verified):
-    """Patch shape only changes which tile is staged, never the value: bit-identical outputs (one thread per
-    point; the warp-per-point form adds its partial sums in a fixed lane order, so it is layout-free too)."""
-    _require(verified, "slice_staged")
+    """Patch shape only changes which tile is staged, never the value: bit-identical outputs (the warp-per-point
+    form adds its partial sums in a fixed lane order, so it is layout-free)."""
+    _require(verified, "slice_coop")
     cfg, model, pix, refs, _ = tiny
     outs = []
     for layout in ((1, 32, 32), (4, 16, 16), (0, 0, 0)):
         ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
-        ctx.spf_set_option("slice_impl", 0)
+        ctx.spf_set_option("slice_impl", 2)
         ctx.spf_set_detector_layout(*layout)
         ctx.spf_prepare_model(_dev(model))
         outs.append(ctx.spf_slice(_dev(refs[:8]), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy())
@@ -80,7 +80,7 @@ def test_staged_slice_equals_the_layout_free_result(spf, tiny, verified):
 @pytest.mark.parametrize("variant,impl", STAGED)
 @pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9)])
 def test_staged_slice_general_model(spf, verified, N, eps, variant, impl):
-    """Non-even model (complex fine grid), even and odd N, w = 7 and w = 10 (w = 10 runs one thread per point)."""
+    """Non-even model (complex fine grid), even and odd N, w = 7 and w = 10 (w = 10 gathers from global memory with the 16-cell window)."""
     _require(verified, variant)
     rng = np.random.default_rng(4)
     A = rng.standard_normal((N, N, N)).astype(np.float32)

@@ -36,7 +36,7 @@ def sim():
     L.hostsim_cell.argtypes = [C.c_double, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
     L.hostsim_slice_blocks.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_long,
                                        C.c_void_p, C.c_long, C.c_void_p, C.c_long, C.c_int, C.c_uint, C.c_void_p, C.c_void_p]
-    L.hostsim_tile_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_int, C.c_void_p]
+    L.hostsim_tile_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_void_p]
     L.hostsim_scatter_model.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]
     L.hostsim_relayout.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
     L.hostsim_count_uneven.argtypes = [C.c_void_p, C.c_int]
@@ -212,7 +212,7 @@ def test_paper_scale_sampled_vs_oracle(sim):
 
 
 # ------------------------------------------------------------------------------------------------
-# staged kernels (slice_impl 0 and 2): block-level replay of the tile staging and of the warp-per-point gather
+# staged kernel (slice_impl 2) and its global-memory twin (3): block-level replay of the tile staging and of the warp-per-point gather
 # ------------------------------------------------------------------------------------------------
 def _patch_table(sim, panels, rows, cols, P):
     """The table spf_slice itself builds (build_patch_table, spf_slice_math.cuh), through the host-compiled header."""
@@ -248,14 +248,14 @@ def _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, quats, pix, table, coo
     out = np.full((quats.shape[0], pix.shape[0]), np.nan + 0j, np.complex64)
     stats = np.zeros(3, np.int64)
     if cap is None:
-        cap = 72 * 1024 if w == 10 else (48 if coop else 36) * 1024 * (1 if is_real else 2)    # launch_slice (spf_slice.cu)
+        cap = 48 * 1024 * (1 if is_real else 2)    # launch_slice (spf_slice.cu)
     sim.hostsim_slice_blocks(grid.ctypes.data, int(is_real), npad, sz, nf, halo, w, quats.ctypes.data, quats.shape[0],
                              pix.ctypes.data, pix.shape[0], table.ctypes.data, len(table) // 128, int(coop), cap,
                              out.ctypes.data, stats.ctypes.data)
     return out, stats
 
 
-@pytest.mark.parametrize("coop,is_real,layout", [(1, 1, True), (1, 0, True), (0, 1, True), (1, 1, False), (0, 0, False),
+@pytest.mark.parametrize("coop,is_real,layout", [(1, 1, True), (1, 0, True), (1, 1, False), (1, 0, False),
                                                  (2, 1, True), (2, 0, False)])
 def test_staged_block_replay_tiny_full_vs_oracle(sim, coop, is_real, layout):
     """Tiny through the staged data path: every block's tile image holds NaN wherever no TMA copy writes,
@@ -291,10 +291,9 @@ def test_staged_block_replay_ragged_patch_and_complex_general_model(sim):
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
     table = _patch_table(sim, 0, 0, 0, 200)
     ref = orc.slice_points(A, refs, pix)
-    for coop in (0, 1):
-        c, stats = _slice_blocks(sim, g, 0, npad, sz, nf, halo, w, refs, pix, table, coop)
-        assert np.isfinite(c.view(np.float32)).all() and stats[0] > 0
-        assert _rel(c, ref) <= SLICE_TOL
+    c, stats = _slice_blocks(sim, g, 0, npad, sz, nf, halo, w, refs, pix, table, 1)
+    assert np.isfinite(c.view(np.float32)).all() and stats[0] > 0
+    assert _rel(c, ref) <= SLICE_TOL
 
 
 def test_warp_per_point_fallback_blocks_equal_the_staged_ones(sim):
@@ -313,24 +312,6 @@ def test_warp_per_point_fallback_blocks_equal_the_staged_ones(sim):
         direct, st3 = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, 2)
         assert st1[0] > 0 and st2[0] == 0 and st3[0] == 0
         assert np.array_equal(staged, forced) and np.array_equal(staged, direct)
-
-
-def test_staged_block_replay_wide_kernel(sim):
-    """w = 10 (eps = 1e-9) through the staged one-thread-per-point path with its 72 KB tile, real and complex grid."""
-    rng = np.random.default_rng(8)
-    N = 21
-    w, nf, halo = _plan(N, 1e-9)
-    assert w == 10
-    pix = make_detector(1, 64)                    # 0.6 fine cells per pixel: an 8 x 16 patch spans about 20 cells
-    refs = random_quaternions(3, seed=31)
-    table = _patch_table(sim, 1, 64, 64, 4096)
-    for is_real in (1, 0):
-        A = make_model(N, 12, 5.0) if is_real else rng.standard_normal((N, N, N)).astype(np.float32)
-        g, npad, sz = _padded_grid(sim, A, w, nf, halo)
-        c, stats = _slice_blocks(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, table, 0)
-        assert np.isfinite(c.view(np.float32)).all() and stats[0] > 0
-        ref = orc.slice_points(A, refs, pix)
-        assert _rel(c.real if is_real else c, ref.real if is_real else ref) <= SLICE_TOL
 
 
 def test_wide_warp_per_point_replay(sim):
@@ -374,38 +355,39 @@ def test_staged_block_replay_paper_scale_sampled(sim):
 
 
 def test_tile_geometry_menu_and_bank_rule(sim):
-    """tile_geom: an accepted box is on the tensor-map menu, covers the points' footprint (plus the 8 x 8 window's
-    spare row and cell in the cooperative form), keeps x-planes 128-byte aligned, fits the capacity, and in the
-    cooperative form has a row pitch of 8 mod 16 cells -- the four rows a warp reads at once then fall into four
-    disjoint groups of 8 banks (real grid) or, per half-warp, two disjoint groups of 16 banks (complex grid)."""
+    """tile_geom: an accepted box is on the tensor-map menu, covers the points' footprint plus the 8 x 8 window's
+    spare row and cell, keeps x-planes 128-byte aligned, fits the capacity, and has a row pitch of 8 mod 16 cells --
+    the four rows a warp reads at once then fall into four disjoint groups of 8 banks (real grid) or, per
+    half-warp, two disjoint groups of 16 banks (complex grid).  w > 8 is never staged."""
     out = (C.c_int * 4)()
-    for coop in (0, 1):
-        for cell in (4, 8):
-            cap = (48 if coop else 36) * 1024 * (cell // 4)
-            for Lx in (7, 13, 22, 30):
-                for Ly in range(7, 45):
-                    for Lz in range(7, 45):
-                        sim.hostsim_tile_geom(Lx, Ly, Lz, 7, cell, cap, coop, out)
-                        by, bz, S1, ok = out[0], out[1], out[2], out[3]
-                        if not ok:
-                            assert by > 40 or bz > 40 or Lz + coop > 40 or Lx * S1 * cell > cap
-                            continue
-                        assert by in range(8, 41, 4) and bz in range(8, 41, 4)
-                        assert by >= Ly + coop and bz >= Lz + coop and S1 >= by * bz and (S1 * cell) % 128 == 0
-                        assert Lx * S1 * cell <= cap
-                        if coop:
-                            assert bz % 16 == 8
-                            if cell == 4:
-                                banks = sorted((h * bz + k) % 32 for h in range(4) for k in range(8))
-                                assert banks == list(range(32))
-                            else:
-                                for half in (0, 2):
-                                    words = sorted(((h * bz + k) * 2 + e) % 32 for h in (half, half + 1) for k in range(8) for e in (0, 1))
-                                    assert words == list(range(32))
+    for cell in (4, 8):
+        cap = 48 * 1024 * (cell // 4)
+        sim.hostsim_tile_geom(13, 20, 20, 10, cell, cap, out)
+        assert out[3] == 0                      # the 8 x 8 window does not cover a 10-wide kernel
+        for Lx in (7, 13, 22, 30):
+            for Ly in range(7, 45):
+                for Lz in range(7, 45):
+                    sim.hostsim_tile_geom(Lx, Ly, Lz, 7, cell, cap, out)
+                    by, bz, S1, ok = out[0], out[1], out[2], out[3]
+                    if not ok:
+                        assert by > 40 or bz > 40 or Lz + 1 > 40 or Lx * S1 * cell > cap
+                        continue
+                    assert by in range(8, 41, 4) and bz in range(8, 41, 4)
+                    assert by >= Ly + 1 and bz >= Lz + 1 and S1 >= by * bz and (S1 * cell) % 128 == 0
+                    assert Lx * S1 * cell <= cap
+                    assert bz % 16 == 8
+                    if cell == 4:
+                        banks = sorted((h * bz + k) % 32 for h in range(4) for k in range(8))
+                        assert banks == list(range(32))
+                    else:
+                        for half in (0, 2):
+                            words = sorted(((h * bz + k) * 2 + e) % 32 for h in (half, half + 1) for k in range(8) for e in (0, 1))
+                            assert words == list(range(32))
 
 
 def test_bank_conflicts_thread_per_point_vs_warp_per_point():
-    """Why slice_impl 2 exists.  With one thread per point the 32 lanes of a warp read, at
+    """Why slice_impl 2 gathers with a WARP per point, and why the round-1 one-thread-per-point staged form (variant 0)
+    was deleted.  With one thread per point the 32 lanes of a warp read, at
     every tap, 32 words whose tile addresses follow the rotated pixel lattice -- generic orientations spread them
     over the 32 banks like random throws, and the load replays max-bank-multiplicity times.  Paper-scale
     geometry, seeded orientations: the mean replay factor is above 3, i.e. 343 x 3.5 / 32 = 38 shared-memory
