@@ -235,7 +235,9 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
     if (threadIdx.x == 0) {
         assert((smem_base & 1023u) == 0u);                                           // SWIZZLE_128B atom alignment
         assert(smem_base + ST * Cfg::STAGE_BYTES + SMEM_AUX <= ptx::smem_u32(smem_raw) + (uint32_t)Cfg::SMEM_BYTES);
-        assert(((smem_base + ST * Cfg::STAGE_BYTES) >> 4) < (1u << 14));            // 14-bit start-address field of the UMMA descriptor
+        // 14-bit start-address field of the UMMA descriptor (the window offset; in a CTA pair the odd CTA's shared
+        // addresses carry its rank above bit 18, which umma_desc_sw128 masks off)
+        assert((((smem_base & 0x3FFFFu) + ST * Cfg::STAGE_BYTES) >> 4) <= (1u << 14));
         assert((bar_full & 7u) == 0u);
         assert(gridDim.x % CG == 0 && a.chunk_kb >= 1);
     }

@@ -1,0 +1,256 @@
+"""The kernels' OWN SOURCE executed on the CPU under the functional emulator of tests/emu/, against the oracle.
+
+tests/emu/build_emu.py compiles paper_2109_05339_b200/csrc/*.cu with g++ after a mechanical rewrite (launch syntax,
+dynamic shared memory, inline-PTX wrappers replaced by functional stand-ins) and links it with a fiber scheduler that
+runs every CUDA thread of a block -- or of a CTA pair -- cooperatively: block barriers, warp shuffles and votes,
+mbarrier phases and transaction counts, deferred TMA copies with the 128-byte swizzle, a software TMEM and
+tcgen05.mma reading its operands through the kernels' own shared-memory descriptors.  The tests below call the
+library's C ABI exactly as the GPU tests do (tests/test_gpu_parity.py, tests/test_gpu_variants.py), at sizes the
+emulator finishes in seconds, and hold the results to the same bars: slices relative L2 <= 1e-5, distances <= 1e-4,
+argmin exact outside near-ties.
+
+What this is: evidence, obtainable without a GPU, that the kernels' index arithmetic, barrier protocols, pipelines,
+descriptors and epilogues are self-consistent and compute the method -- for the library's
+default kernels AND for the TMA / tcgen05 variants.  What it is not: GPU parity.  The emulator implements the
+programming model as tests/emu/ptx_emu.cuh states it; whether sm_100a agrees is only shown by `-m gpu` on a B200.
+Poisoned memory (NaN in fresh device allocations, in shared memory and in TMEM) turns a read of anything the
+kernels did not write into a NaN result, and the emulator faults on misaligned TMA destinations, uninitialised
+barriers, TMEM accesses outside the warp's lane quadrant or the allocation, and TMEM left allocated at exit.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from spf_inputs import (CONFIGS, make_model, make_detector, random_quaternions, planted_truth_quaternions, photon_scale,
+                        poisson_images)
+
+sys.path.insert(0, os.path.join(os.path.dirname(os.path.abspath(__file__)), "emu"))
+import emu_binding as eb  # noqa: E402
+from emu_binding import EmuContext, EmuError, SPF_OUT_COMPLEX, SPF_OUT_INTENSITY  # noqa: E402
+
+SLICE_TOL = 1e-5
+DIST_TOL = 1e-4
+SLICERS = [(1, "thread-per-point global gather (library default)"), (3, "warp-per-point from global memory"),
+           (2, "warp-per-point from a TMA-staged tile")]
+MATCHERS = ["simt", "cg1", "cg2"]
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    cfg = CONFIGS["tiny"]
+    model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(cfg.M, seed=2)
+    return cfg, model, pix, refs, orc.slice_points(model, refs, pix)
+
+
+def _matcher(ctx, variant):
+    ctx.set_option("match_impl", 1 if variant == "simt" else 0)
+    ctx.set_option("match_cta_group", 2 if variant == "cg2" else 1)
+
+
+def _check_match(bi, bd, I, S, mask=None):
+    oi, od, osd, _ = orc.match(I, S, mask)
+    tol = DIST_TOL * np.maximum(od, 1e-30)
+    assert np.all(np.isfinite(bd))
+    assert np.all(np.abs(bd - od) <= tol + 1e-6 * (od == 0)), "max rel %.3e" % float(np.max(np.abs(bd - od) / np.maximum(od, 1e-30)))
+    near = (osd - od) <= tol
+    assert np.all((bi == oi) | near), (bi, oi)
+    return float(np.max(np.abs(bd - od) / np.maximum(od, 1e-30)))
+
+
+# --------------------------------------------------------------------------------- a1 + a2: spf_prepare_model
+
+@pytest.mark.parametrize("N", [21, 16])
+def test_emulated_prepare_is_the_nudft_of_the_deapodised_model(N):
+    """k_check_even, k_deapod_pad, (DFT stub in place of cuFFT), k_relayout: b_l against the oracle's NUDFT of A p p p."""
+    rng = np.random.default_rng(3)
+    A = make_model(21, 12, 5.0) if N == 21 else rng.standard_normal((N, N, N)).astype(np.float32)
+    ctx = EmuContext(N, eps=1e-6)
+    ctx.prepare_model(A)
+    assert ctx.info.grid_is_real == (1 if N == 21 else 0)
+    nf = ctx.info.n_fine
+    b = ctx.fine_grid()
+    p = ctx.deapodisation()
+    Ap = (A.astype(np.float64) * p[:, None, None] * p[None, :, None] * p[None, None, :]).astype(np.float32)
+    l = rng.integers(0, nf, size=(200, 3))
+    ref = orc.nudft(Ap, 2 * np.pi * l / nf)
+    assert _rel(b[l[:, 0], l[:, 1], l[:, 2]], ref) <= 2e-6
+
+
+# --------------------------------------------------------------------------------- a3-a5: spf_slice
+
+@pytest.mark.parametrize("impl,what", SLICERS)
+@pytest.mark.parametrize("force_complex,layout", [(0, True), (1, False)])
+def test_emulated_slice_tiny_vs_oracle(tiny, impl, what, force_complex, layout):
+    cfg, model, pix, refs, c_ref = tiny
+    m = 12                                       # 12 orientations x 1,024 pixels: 96 blocks of 128 points
+    ctx = EmuContext(cfg.N, eps=cfg.eps)
+    if layout:
+        ctx.set_detector_layout(1, 32, 32)
+    ctx.set_option("slice_impl", impl)
+    ctx.set_option("force_complex_grid", force_complex)
+    ctx.prepare_model(model)
+    eb.counters()
+    c = ctx.slice(refs[:m], pix, SPF_OUT_COMPLEX)
+    n = eb.counters()
+    assert np.isfinite(c.view(np.float32)).all()
+    assert _rel(c, c_ref[:m]) <= SLICE_TOL
+    assert (n["tma_copies"] > 0) == (impl == 2), n          # the staged variant really stages, the others never touch TMA
+    s = ctx.slice(refs[:m], pix, SPF_OUT_INTENSITY, scale=2.5)
+    assert np.array_equal(s, np.float32(2.5) * c.real.astype(np.float32))
+
+
+def test_emulated_slicers_agree_bit_for_bit_where_they_should(tiny):
+    """Variants 2 and 3 walk the same window with the same weights in the same order: identical bits; and the result
+    does not depend on how pixels are grouped into patches."""
+    cfg, model, pix, refs, _ = tiny
+    outs = {}
+    for impl in (2, 3):
+        for layout in ((1, 32, 32), (4, 16, 16), (0, 0, 0)):
+            ctx = EmuContext(cfg.N, eps=cfg.eps)
+            ctx.set_detector_layout(*layout)
+            ctx.set_option("slice_impl", impl)
+            ctx.prepare_model(model)
+            outs[(impl, layout)] = ctx.slice(refs[:4], pix, SPF_OUT_COMPLEX)
+    first = outs[(2, (1, 32, 32))]
+    for k, v in outs.items():
+        assert np.array_equal(v, first), k
+
+
+@pytest.mark.parametrize("impl", [1, 2, 3])
+@pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9), (12, 1e-4)])
+def test_emulated_slice_general_model_widths_and_even_n(impl, N, eps):
+    """Non-even model (complex grid), even N, w = 7 / 10 / 5 (run-time width: reference gather only)."""
+    rng = np.random.default_rng(4)
+    A = rng.standard_normal((N, N, N)).astype(np.float32)
+    pix = make_detector(1, 16)
+    refs = random_quaternions(5, seed=31)
+    ctx = EmuContext(N, eps=eps)
+    ctx.set_option("slice_impl", impl)
+    ctx.set_detector_layout(1, 16, 16)
+    ctx.prepare_model(A)
+    assert ctx.info.grid_is_real == 0
+    c = ctx.slice(refs, pix, SPF_OUT_COMPLEX)
+    assert _rel(c, orc.slice_points(A, refs, pix)) <= max(SLICE_TOL, 10 * eps)
+
+
+@pytest.mark.parametrize("impl", [1, 2, 3])
+def test_emulated_slice_edge_cases(tiny, impl):
+    cfg, model, pix, refs, c_ref = tiny
+    ctx = EmuContext(cfg.N, eps=cfg.eps)
+    ctx.set_option("slice_impl", impl)
+    with pytest.raises(EmuError) as e:
+        ctx.slice(refs[:1], pix)
+    assert e.value.status == -4                                     # SPF_ESTATE before spf_prepare_model
+    ctx.prepare_model(model)
+    assert ctx.slice(refs[:0], pix).shape == (0, 1024) and ctx.slice(refs[:2], pix[:0]).shape == (2, 0)
+    # ragged P, unnormalised quaternions, q outside [-pi, pi], points at the very edge of the period
+    c = ctx.slice((3.0 * refs[:3]).astype(np.float32), pix[:777], SPF_OUT_COMPLEX)
+    assert _rel(c, c_ref[:3, :777]) <= SLICE_TOL
+    ident = np.array([[1, 0, 0, 0]], np.float32)
+    far = (pix[:200].astype(np.float64) + 2 * np.pi * np.array([1, -1, 2])).astype(np.float32)
+    assert _rel(ctx.slice(ident, far, SPF_OUT_COMPLEX), orc.slice_points(model, ident, far)) <= SLICE_TOL
+    edge = np.array([[np.pi, -np.pi, 0.0], [-np.pi, np.pi, np.pi], [3.14159, 3.14159, -3.14159]], np.float32)
+    # |c| ~ 1e-5 at the Nyquist edge against an rms of ~36 over the slices: the bar is absolute (reading s15)
+    err = np.max(np.abs(ctx.slice(ident, edge, SPF_OUT_COMPLEX) - orc.slice_points(model, ident, edge)))
+    assert err <= SLICE_TOL * np.sqrt(np.mean(np.abs(c_ref) ** 2))
+
+
+# --------------------------------------------------------------------------------- a6-a8: spf_match
+
+@pytest.mark.parametrize("variant", MATCHERS)
+@pytest.mark.parametrize("n_img,M,P,masked", [(16, 64, 1024, False), (5, 300, 1000, True), (130, 257, 192, False), (300, 513, 320, True)])
+def test_emulated_match_vs_oracle_ragged_sizes(variant, n_img, M, P, masked):
+    rng = np.random.default_rng(n_img * 7 + M)
+    S = (rng.random((M, P)) * rng.random((M, 1)) * 3).astype(np.float32)
+    I = rng.poisson(S[rng.integers(0, M, n_img)]).astype(np.float32)
+    mask = (rng.random(P) > 0.2).astype(np.uint8) if masked else None
+    ctx = EmuContext(8, sm_count=4)              # 4 SMs: 4 (2) persistent clusters, so clusters take several tiles
+    _matcher(ctx, variant)
+    eb.counters()
+    bi, bd, prods = ctx.match(I, S, mask)
+    n = eb.counters()
+    assert prods == (0 if variant == "simt" else 2)              # photon counts: one fp16 image plane
+    assert (n["mmas"] > 0) == (variant != "simt") and (n["tma_copies"] > 0) == (variant != "simt")
+    _check_match(bi, bd, I, S, mask)
+    ri, rd, dist = ctx.match_reference(I, S, mask)               # the independent CUDA-core reference kernels
+    assert np.allclose(dist, orc.distances(I, S, mask), rtol=1e-6)
+
+
+@pytest.mark.parametrize("variant", ["cg1", "cg2"])
+@pytest.mark.parametrize("chunk", [1, 3, 0])
+def test_emulated_tcgen05_epilogue_without_refinement(variant, chunk):
+    """The contraction's own a_i + b_m - 2 G (match_refine = 0), with the accumulator drained every 1 or 3 K blocks
+    (both TMEM stages, many hand-overs between the MMA issuer and the epilogue warps) or once (chunk 0)."""
+    rng = np.random.default_rng(11)
+    n_img, M, P = 140, 300, 448
+    S = (rng.random((M, P)) * 2).astype(np.float32)
+    I = rng.poisson(S[rng.integers(0, M, n_img)]).astype(np.float32)
+    ctx = EmuContext(8, sm_count=2)
+    _matcher(ctx, variant)
+    ctx.set_option("match_refine", 0)
+    ctx.set_option("match_chunk_kblocks", chunk)
+    bi, bd, prods = ctx.match(I, S)
+    assert prods == 2
+    worst = _check_match(bi, bd, I, S)
+    assert worst < 2e-5
+
+
+@pytest.mark.parametrize("variant", MATCHERS)
+def test_emulated_match_planted_ties_and_general_values(variant):
+    rng = np.random.default_rng(17)
+    M, P = 200, 640
+    S = rng.random((M, P)).astype(np.float32)
+    S[150] = S[20]                                               # exact duplicate: the lowest index must win
+    planted = np.array([20, 0, 199, 77])
+    I = S[planted].copy()                                        # non-integer images: two fp16 image planes, 3 products
+    ctx = EmuContext(8, sm_count=4)
+    _matcher(ctx, variant)
+    bi, bd, prods = ctx.match(I, S)
+    assert list(bi) == list(planted) and prods == (0 if variant == "simt" else 3)
+    nrm = (I.astype(np.float64) ** 2).sum(1) + (S[planted].astype(np.float64) ** 2).sum(1)
+    assert np.all(np.abs(bd) <= 1e-6 * nrm)                      # reading s14, the noise-free case
+    # counts above 2,048 (not exact in one fp16 term) at d ~ 3e-4 of the norms: same 1e-4 d bar (conditioning + refinement)
+    S3 = (3000.0 * S).astype(np.float32)
+    I2 = rng.poisson(3000.0 * S[rng.integers(0, M, 9)]).astype(np.float32)
+    bi, bd, _ = ctx.match(I2, S3)
+    _check_match(bi, bd, I2, S3)
+    bi4, bd4, _ = ctx.match(4 * I2, 4 * S3)                      # power-of-two scaling passes through exactly
+    assert np.array_equal(bi4, bi) and np.allclose(bd4, 16 * bd, rtol=1e-6)
+    perm = rng.permutation(M)                                    # permuting the reference set permutes the answer
+    bip, bdp, _ = ctx.match(I2, S3[perm])
+    assert np.array_equal(perm[bip], bi) and np.allclose(bdp, bd, rtol=1e-5)
+    with pytest.raises(EmuError):
+        ctx.match(I, S[:0])
+
+
+# --------------------------------------------------------------------------------- the whole path
+
+@pytest.mark.parametrize("impl,variant", [(1, "simt"), (3, "simt"), (2, "cg1"), (2, "cg2")])
+def test_emulated_end_to_end_tiny_poisson(tiny, impl, variant):
+    """Tiny (BASELINE.json:configs[0]) end to end: everything from the oracle on one side, everything from the
+    emulated kernels on the other -- the library defaults, and the TMA-staged slicer with each tcgen05 matcher."""
+    cfg, model, pix, refs, c_ref = tiny
+    truth, _ = planted_truth_quaternions(cfg.n_img, refs)
+    alpha = photon_scale(c_ref.real, None, cfg.photons)
+    images = poisson_images(alpha * orc.slice_points(model, truth, pix).real)
+    ctx = EmuContext(cfg.N, eps=cfg.eps)
+    ctx.set_detector_layout(1, 32, 32)
+    ctx.set_option("slice_impl", impl)
+    _matcher(ctx, variant)
+    ctx.prepare_model(model)
+    slices = ctx.slice(refs, pix, SPF_OUT_INTENSITY, scale=alpha)
+    bi, bd, _ = ctx.match(images, slices)
+    oi, od, osd, _ = orc.match(images, alpha * c_ref.real)        # the oracle's own fp64 slices
+    near = (osd - od) <= DIST_TOL * od
+    assert np.all((bi == oi) | near) and np.all(np.abs(bd - od) <= DIST_TOL * od)
+    hi, hd, hs = ctx.orientation_match_host(model, refs, pix, images, scale=alpha)     # the host-buffer entry point
+    assert np.array_equal(hi, bi) and np.array_equal(hd, bd) and np.array_equal(hs, slices)
