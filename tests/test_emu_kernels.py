@@ -181,8 +181,10 @@ def test_emulated_match_vs_oracle_ragged_sizes(variant, n_img, M, P, masked):
     assert prods == (0 if variant == "simt" else 2)              # photon counts: one fp16 image plane
     assert (n["mmas"] > 0) == (variant != "simt") and (n["tma_copies"] > 0) == (variant != "simt")
     _check_match(bi, bd, I, S, mask)
-    ri, rd, dist = ctx.match_reference(I, S, mask)               # the independent CUDA-core reference kernels
-    assert np.allclose(dist, orc.distances(I, S, mask), rtol=1e-6)
+    if n_img * M <= 2000:                                        # the independent CUDA-core reference kernels (one block per
+        ri, rd, dist = ctx.match_reference(I, S, mask)           # pair: only the small cases are affordable under emulation)
+        assert np.allclose(dist, orc.distances(I, S, mask), rtol=1e-6)
+        assert np.array_equal(ri, bi) or variant != "simt"
 
 
 @pytest.mark.parametrize("variant", ["cg1", "cg2"])
