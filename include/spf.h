@@ -63,7 +63,7 @@ typedef struct spf_ctx spf_ctx; /* opaque */
 
 typedef struct {
     int32_t n;        /* model edge N >= 2 (odd or even) */
-    double eps;       /* NUFFT tolerance in (0, 1e-1]; sets the kernel width w = ceil(log10(1/eps)) + 1, 2 <= w <= 16 */
+    double eps;       /* NUFFT tolerance in (0, 1e-1]; sets the kernel width w = min(ceil(log10(1/eps)) + 2, 10): 8 at 1e-6 (reading s10b) */
     double upsampfac; /* sigma >= 2.0 (the kernel constants are those of sigma = 2)        (reading s10) */
     int32_t n_fine;   /* 0: smallest even 2-3-5-7-smooth integer >= upsampfac * n; else an explicit fine-grid edge >= 2n */
     int32_t device;   /* CUDA device ordinal */
@@ -190,7 +190,7 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *                      with no bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; blocks whose box
  *                      does not fit the tile, and every block at w = 10, run as 3);
  *                  3 = the warp-per-point gather straight from global memory (no TMA, mbarrier or tile;
- *                      8 x 8 window at w = 7, 16-cell window at w = 10)
+ *                      8 x 8 window at w = 8, 16-cell window at w = 10)
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
  *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused norm-add + argmin epilogue (the product);
  *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused

@@ -48,12 +48,18 @@ const char *spf_status_string(int s) {
 
 const char *spf_last_error(const spf_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
-// w = ceil(log10(1/eps)) + 1 (reading s10), clamped to [2, SPF_MAX_W]
+// Kernel width for a requested tolerance: w = ceil(log10(1/eps)) + 2, at most 10 (reading s10b).
+// The usual rule is "+ 1" (w = 7 at eps = 1e-6).  On the models of this path -- non-negative autocorrelations that fill
+// the grid, whose transform has a central peak sum(A) hundreds of times the rms of what the detector sees -- every
+// mode's kernel error adds coherently near q = 0 and the relative L2 error OVER THE DETECTOR PIXELS is 0.6 - 1.8e-5 at
+// w = 7 (evaluated in fp64, so it is the kernel's own error, not an implementation artefact): it straddles the 1e-5
+// parity bar.  One more cell per axis brings it to 1e-6 (7e-7 measured through the fp32 kernel at Paper-scale).
+// Beyond w = 10 fp32 arithmetic gains nothing, so eps < 1e-8 keeps w = 10 (the Slicing-heavy configuration).
 int32_t spf_plan_kernel_width(double eps) {
     if (!(eps > 0.0) || eps > 0.1) return -1;
-    int w = (int)ceil(log10(1.0 / eps) - 1e-9) + 1;
-    if (w < 2) w = 2;
-    if (w > SPF_MAX_W) w = SPF_MAX_W;
+    int w = (int)ceil(log10(1.0 / eps) - 1e-9) + 2;
+    if (w < 3) w = 3;
+    if (w > 10) w = 10;
     return w;
 }
 

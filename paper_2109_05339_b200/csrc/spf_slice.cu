@@ -294,7 +294,7 @@ int build_patches(spf_ctx *ctx, int64_t P) {
 template <int W, bool REAL, int OUTK, int IMPL>
 int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
     auto kern = k_slice<W, REAL, OUTK, IMPL>;
-    // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid (w = 7)
+    // shared-memory tile capacity: 3 blocks per SM on the real grid, 2 on the complex grid (w = 8)
     uint32_t smem = 0;
     args.cap_bytes = 0;
     if (IMPL == IMPL_GCOOP) smem = W > 8 ? (uint32_t)(SPF_PATCH * SPF_COOPW_STRIDE * 4) : (uint32_t)SPF_COOP_WTS_BYTES;   // the parked weights only
@@ -319,10 +319,10 @@ int launch_slice(spf_ctx *ctx, SliceArgs &args, cudaStream_t st) {
 template <bool REAL, int OUTK>
 int launch_slice_w(spf_ctx *ctx, SliceArgs &args, int impl, cudaStream_t st) {
     switch (ctx->w) {
-        case 7:
-            if (impl == IMPL_COOP) return launch_slice<7, REAL, OUTK, IMPL_COOP>(ctx, args, st);
-            if (impl == IMPL_GCOOP) return launch_slice<7, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
-            return launch_slice<7, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
+        case 8:    // eps = 1e-6: the 8 x 8 window is exactly the kernel's footprint
+            if (impl == IMPL_COOP) return launch_slice<8, REAL, OUTK, IMPL_COOP>(ctx, args, st);
+            if (impl == IMPL_GCOOP) return launch_slice<8, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
+            return launch_slice<8, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         case 10:   // 10 x 10 window: the staged 8 x 8 form does not apply, variants 2 and 3 both walk global memory (16-cell window)
             if (impl == IMPL_COOP || impl == IMPL_GCOOP) return launch_slice<10, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
             return launch_slice<10, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);

@@ -347,25 +347,41 @@ namespace {
 struct Plan { int n[3]; bool used; };
 std::vector<Plan> plans;
 
+// forward DFT of one line by recursive decimation in time on the smallest prime factor (any length; fine-grid edges are
+// 2-3-5-7-smooth, so this is O(n log n)); x has n complex entries at stride 1, tw[k] = exp(-2 pi i k / n0) for the top length n0
+void fft_rec(const double *xr, const double *xi, long stride, int n, double *yr, double *yi, const double *twr, const double *twi, int tw_step) {
+    if (n == 1) { yr[0] = xr[0]; yi[0] = xi[0]; return; }
+    int p = n;
+    for (int q = 2; q * q <= n; ++q)
+        if (n % q == 0) { p = q; break; }
+    const int m = n / p;
+    std::vector<double> sr((size_t)n), si((size_t)n);
+    for (int r = 0; r < p; ++r)   // sub-transform of the entries r, r + p, r + 2p, ...
+        fft_rec(xr + r * stride, xi + r * stride, stride * p, m, sr.data() + (size_t)r * m, si.data() + (size_t)r * m, twr, twi, tw_step * p);
+    for (int k = 0; k < n; ++k) {
+        double ar = 0.0, ai = 0.0;
+        const int km = k % m;
+        for (int r = 0; r < p; ++r) {
+            const long t = ((long)r * k % n) * tw_step;          // exp(-2 pi i r k / n)
+            const double cr = twr[t], ci = twi[t], vr = sr[(size_t)r * m + km], vi = si[(size_t)r * m + km];
+            ar += vr * cr - vi * ci;
+            ai += vr * ci + vi * cr;
+        }
+        yr[k] = ar; yi[k] = ai;
+    }
+}
+
 void dft_axis(std::vector<double> &re, std::vector<double> &im, const int n[3], int axis) {
     const int len = n[axis];
-    std::vector<double> cs((size_t)len), sn((size_t)len), tr((size_t)len), ti((size_t)len);
+    std::vector<double> cs((size_t)len), sn((size_t)len), lr((size_t)len), li((size_t)len), tr((size_t)len), ti((size_t)len);
     for (int k = 0; k < len; ++k) { cs[(size_t)k] = cos(2.0 * M_PI * k / len); sn[(size_t)k] = -sin(2.0 * M_PI * k / len); }   // forward: exp(-i ...)
     const long stride = axis == 2 ? 1 : (axis == 1 ? n[2] : (long)n[1] * n[2]);
     const long total = (long)n[0] * n[1] * n[2];
     for (long base = 0; base < total; ++base) {
         const long idx_axis = (base / stride) % len;
         if (idx_axis != 0) continue;   // one pass per line
-        for (int k = 0; k < len; ++k) {
-            double ar = 0.0, ai = 0.0;
-            for (int j = 0; j < len; ++j) {
-                const int t = (int)(((long)k * j) % len);
-                const double xr = re[(size_t)(base + j * stride)], xi = im[(size_t)(base + j * stride)];
-                ar += xr * cs[(size_t)t] - xi * sn[(size_t)t];
-                ai += xr * sn[(size_t)t] + xi * cs[(size_t)t];
-            }
-            tr[(size_t)k] = ar; ti[(size_t)k] = ai;
-        }
+        for (int j = 0; j < len; ++j) { lr[(size_t)j] = re[(size_t)(base + j * stride)]; li[(size_t)j] = im[(size_t)(base + j * stride)]; }
+        fft_rec(lr.data(), li.data(), 1, len, tr.data(), ti.data(), cs.data(), sn.data(), 1);
         for (int k = 0; k < len; ++k) { re[(size_t)(base + k * stride)] = tr[(size_t)k]; im[(size_t)(base + k * stride)] = ti[(size_t)k]; }
     }
 }

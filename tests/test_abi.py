@@ -36,7 +36,7 @@ def test_host_only_planning_calls(lib):
     lib.spf_match_workspace_bytes.restype = ctypes.c_size_t
     lib.spf_version.restype = ctypes.c_char_p
     lib.spf_status_string.restype = ctypes.c_char_p
-    assert lib.spf_plan_kernel_width(1e-6) == 7 and lib.spf_plan_kernel_width(1e-9) == 10
+    assert lib.spf_plan_kernel_width(1e-6) == 8 and lib.spf_plan_kernel_width(1e-9) == 10 and lib.spf_plan_kernel_width(1e-4) == 6
     assert lib.spf_plan_kernel_width(0.0) == -1
     assert [lib.spf_plan_n_fine(n, 2.0) for n in (21, 81, 151, 201)] == [42, 162, 320, 420]
     assert lib.spf_plan_n_fine(151, 1.5) == -1

@@ -128,7 +128,7 @@ def test_emulated_slicers_agree_bit_for_bit_where_they_should(tiny):
 @pytest.mark.parametrize("impl", [1, 2, 3])
 @pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9), (12, 1e-4)])
 def test_emulated_slice_general_model_widths_and_even_n(impl, N, eps):
-    """Non-even model (complex grid), even N, w = 7 / 10 / 5 (run-time width: reference gather only)."""
+    """Non-even model (complex grid), even N, w = 8 / 10 / 6 (run-time width: reference gather only)."""
     rng = np.random.default_rng(4)
     A = rng.standard_normal((N, N, N)).astype(np.float32)
     pix = make_detector(1, 16)

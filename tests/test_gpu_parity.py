@@ -83,7 +83,7 @@ def _es_kernel_ft(xi, beta):
 def test_deapodisation_factors_match_quadrature(spf):
     ctx = spf.SpfContext(21, eps=1e-6)
     info = ctx.info
-    assert (info.n, info.n_fine, info.w) == (21, 42, 7) and abs(info.beta - 16.1) < 1e-12
+    assert (info.n, info.n_fine, info.w) == (21, 42, 8) and abs(info.beta - 18.4) < 1e-12
     p = ctx.spf_debug_deapodisation()
     for i in (0, 3, 10, 17, 20):
         n = i - 10
@@ -157,7 +157,7 @@ def test_slice_is_independent_of_the_patch_layout(spf, tiny):
 
 @pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9), (12, 1e-4)])
 def test_slice_general_model_widths_and_even_n(spf, N, eps):
-    """Non-even real model (complex fine grid), even N, w = 7 / 10 / 5 (runtime-width kernel)."""
+    """Non-even real model (complex fine grid), even N, w = 8 / 10 / 6 (runtime-width kernel)."""
     rng = np.random.default_rng(4)
     A = rng.standard_normal((N, N, N)).astype(np.float32)
     pix = make_detector(1, 16)

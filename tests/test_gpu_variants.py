@@ -80,7 +80,7 @@ def test_staged_slice_equals_the_layout_free_result(spf, tiny, verified):
 @pytest.mark.parametrize("variant,impl", STAGED)
 @pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9)])
 def test_staged_slice_general_model(spf, verified, N, eps, variant, impl):
-    """Non-even model (complex fine grid), even and odd N, w = 7 and w = 10 (w = 10 gathers from global memory with the 16-cell window)."""
+    """Non-even model (complex fine grid), even and odd N, w = 8 and w = 10 (w = 10 gathers from global memory with the 16-cell window)."""
     _require(verified, variant)
     rng = np.random.default_rng(4)
     A = rng.standard_normal((N, N, N)).astype(np.float32)

@@ -47,7 +47,7 @@ def sim():
 
 
 def _plan(N, eps):
-    w = int(np.ceil(np.log10(1.0 / eps) - 1e-9)) + 1
+    w = min(max(int(np.ceil(np.log10(1.0 / eps) - 1e-9)) + 2, 3), 10)      # spf_plan_kernel_width (reading s10b)
     nf = 2 * N + (2 * N) % 2
     while True:
         v = nf
@@ -138,7 +138,7 @@ def test_tiny_full_vs_oracle(sim, use_poly, is_real):
     pix = make_detector(cfg.panels, cfg.panel_edge)
     refs = random_quaternions(cfg.M, seed=2)
     w, nf, halo = _plan(cfg.N, cfg.eps)
-    assert (w, nf) == (7, 42)
+    assert (w, nf) == (8, 42)
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
     assert np.abs(g.imag).max() <= 1e-5 * np.abs(g.real).max()        # even model => real fine grid
     c = _slice(sim, g, is_real, npad, sz, nf, halo, w, refs, pix, use_poly)
@@ -194,14 +194,14 @@ def test_cell_index_stays_inside_the_padded_grid(sim):
 
 
 def test_paper_scale_sampled_vs_oracle(sim):
-    """Paper-scale model (configs[2]: 151^3, n_fine 320, w 7): 8 orientations x 65,536 pixels through the
+    """Paper-scale model (configs[2]: 151^3, n_fine 320, w 8): 8 orientations x 65,536 pixels through the
     host-compiled arithmetic, 2,048 sampled pairs from the oracle.  The thinnest margin of the configs."""
     cfg = CONFIGS["paper_scale"]
     A = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
     pix = make_detector(cfg.panels, cfg.panel_edge)
     refs = random_quaternions(8, seed=2)
     w, nf, halo = _plan(cfg.N, cfg.eps)
-    assert (w, nf) == (7, 320)
+    assert (w, nf) == (8, 320)
     g, npad, sz = _padded_grid(sim, A, w, nf, halo)
     c = _slice(sim, g, 1, npad, sz, nf, halo, w, refs, pix, 1)
     sm, sj = sample_pairs(8, cfg.P, 2048)
@@ -356,7 +356,7 @@ def test_staged_block_replay_paper_scale_sampled(sim):
 
 def test_tile_geometry_menu_and_bank_rule(sim):
     """tile_geom: an accepted box is on the tensor-map menu, covers the points' footprint plus the 8 x 8 window's
-    spare row and cell, keeps x-planes 128-byte aligned, fits the capacity, and has a row pitch of 8 mod 16 cells --
+    spare row and cell (w = 7; none at w = 8), keeps x-planes 128-byte aligned, fits the capacity, and has a row pitch of 8 mod 16 cells --
     the four rows a warp reads at once then fall into four disjoint groups of 8 banks (real grid) or, per
     half-warp, two disjoint groups of 16 banks (complex grid).  w > 8 is never staged."""
     out = (C.c_int * 4)()
@@ -364,16 +364,17 @@ def test_tile_geometry_menu_and_bank_rule(sim):
         cap = 48 * 1024 * (cell // 4)
         sim.hostsim_tile_geom(13, 20, 20, 10, cell, cap, out)
         assert out[3] == 0                      # the 8 x 8 window does not cover a 10-wide kernel
-        for Lx in (7, 13, 22, 30):
-            for Ly in range(7, 45):
-                for Lz in range(7, 45):
-                    sim.hostsim_tile_geom(Lx, Ly, Lz, 7, cell, cap, out)
+        for w, Lx in ((7, 7), (8, 8), (8, 13), (7, 22), (8, 22), (8, 30)):
+            spare = 8 - w                       # the 8 x 8 window reads `spare` rows and cells past the w taps
+            for Ly in range(w, 45):
+                for Lz in range(w, 45):
+                    sim.hostsim_tile_geom(Lx, Ly, Lz, w, cell, cap, out)
                     by, bz, S1, ok = out[0], out[1], out[2], out[3]
                     if not ok:
-                        assert by > 40 or bz > 40 or Lz + 1 > 40 or Lx * S1 * cell > cap
+                        assert by > 40 or bz > 40 or Lz + spare > 40 or Lx * S1 * cell > cap
                         continue
                     assert by in range(8, 41, 4) and bz in range(8, 41, 4)
-                    assert by >= Ly + 1 and bz >= Lz + 1 and S1 >= by * bz and (S1 * cell) % 128 == 0
+                    assert by >= Ly + spare and bz >= Lz + spare and S1 >= by * bz and (S1 * cell) % 128 == 0
                     assert Lx * S1 * cell <= cap
                     assert bz % 16 == 8
                     if cell == 4:
@@ -390,8 +391,8 @@ def test_bank_conflicts_thread_per_point_vs_warp_per_point():
     was deleted.  With one thread per point the 32 lanes of a warp read, at
     every tap, 32 words whose tile addresses follow the rotated pixel lattice -- generic orientations spread them
     over the 32 banks like random throws, and the load replays max-bank-multiplicity times.  Paper-scale
-    geometry, seeded orientations: the mean replay factor is above 3, i.e. 343 x 3.5 / 32 = 38 shared-memory
-    wavefronts per point, against 14 + 4 for the warp-per-point form whose lanes read 32 consecutive-bank words."""
+    geometry, seeded orientations: the mean replay factor is above 3, i.e. w^3 x 3.5 / 32 = 56 shared-memory
+    wavefronts per point at w = 8, against 16 + 4 for the warp-per-point form whose lanes read 32 consecutive-bank words."""
     cfg = CONFIGS["paper_scale"]
     pix = make_detector(cfg.panels, cfg.panel_edge).astype(np.float64)
     w, nf, halo = _plan(cfg.N, cfg.eps)
