@@ -349,21 +349,22 @@ std::vector<Plan> plans;
 
 // forward DFT of one line by recursive decimation in time on the smallest prime factor (any length; fine-grid edges are
 // 2-3-5-7-smooth, so this is O(n log n)); x has n complex entries at stride 1, tw[k] = exp(-2 pi i k / n0) for the top length n0
-void fft_rec(const double *xr, const double *xi, long stride, int n, double *yr, double *yi, const double *twr, const double *twi, int tw_step) {
+template <class R>
+void fft_rec(const R *xr, const R *xi, long stride, int n, R *yr, R *yi, const R *twr, const R *twi, int tw_step) {
     if (n == 1) { yr[0] = xr[0]; yi[0] = xi[0]; return; }
     int p = n;
     for (int q = 2; q * q <= n; ++q)
         if (n % q == 0) { p = q; break; }
     const int m = n / p;
-    std::vector<double> sr((size_t)n), si((size_t)n);
+    std::vector<R> sr((size_t)n), si((size_t)n);
     for (int r = 0; r < p; ++r)   // sub-transform of the entries r, r + p, r + 2p, ...
         fft_rec(xr + r * stride, xi + r * stride, stride * p, m, sr.data() + (size_t)r * m, si.data() + (size_t)r * m, twr, twi, tw_step * p);
     for (int k = 0; k < n; ++k) {
-        double ar = 0.0, ai = 0.0;
+        R ar = 0, ai = 0;
         const int km = k % m;
         for (int r = 0; r < p; ++r) {
             const long t = ((long)r * k % n) * tw_step;          // exp(-2 pi i r k / n)
-            const double cr = twr[t], ci = twi[t], vr = sr[(size_t)r * m + km], vi = si[(size_t)r * m + km];
+            const R cr = twr[t], ci = twi[t], vr = sr[(size_t)r * m + km], vi = si[(size_t)r * m + km];
             ar += vr * cr - vi * ci;
             ai += vr * ci + vi * cr;
         }
@@ -371,10 +372,11 @@ void fft_rec(const double *xr, const double *xi, long stride, int n, double *yr,
     }
 }
 
-void dft_axis(std::vector<double> &re, std::vector<double> &im, const int n[3], int axis) {
+template <class R>
+void dft_axis(std::vector<R> &re, std::vector<R> &im, const int n[3], int axis) {
     const int len = n[axis];
-    std::vector<double> cs((size_t)len), sn((size_t)len), lr((size_t)len), li((size_t)len), tr((size_t)len), ti((size_t)len);
-    for (int k = 0; k < len; ++k) { cs[(size_t)k] = cos(2.0 * M_PI * k / len); sn[(size_t)k] = -sin(2.0 * M_PI * k / len); }   // forward: exp(-i ...)
+    std::vector<R> cs((size_t)len), sn((size_t)len), lr((size_t)len), li((size_t)len), tr((size_t)len), ti((size_t)len);
+    for (int k = 0; k < len; ++k) { cs[(size_t)k] = (R)cos(2.0 * M_PI * k / len); sn[(size_t)k] = (R)-sin(2.0 * M_PI * k / len); }   // forward: exp(-i ...)
     const long stride = axis == 2 ? 1 : (axis == 1 ? n[2] : (long)n[1] * n[2]);
     const long total = (long)n[0] * n[1] * n[2];
     for (long base = 0; base < total; ++base) {
@@ -398,9 +400,19 @@ cufftResult cufftExecC2C(cufftHandle plan, cufftComplex *in, cufftComplex *out, 
     if (plan < 0 || plan >= (int)plans.size() || dir != CUFFT_FORWARD) return 1;
     const int *n = plans[(size_t)plan].n;
     const size_t total = (size_t)n[0] * n[1] * n[2];
+    // fp64 by default (the stub then adds no error of its own); SPF_EMU_FFT32=1 runs the same transform in fp32, the
+    // arithmetic cuFFT uses, to see what an fp32 FFT's rounding does to the slices (tests/test_emu_kernels.py)
+    const char *f32 = getenv("SPF_EMU_FFT32");
+    if (f32 && f32[0] == '1') {
+        std::vector<float> re(total), im(total);
+        for (size_t i = 0; i < total; ++i) { re[i] = in[i].x; im[i] = in[i].y; }
+        for (int axis = 0; axis < 3; ++axis) dft_axis<float>(re, im, n, axis);
+        for (size_t i = 0; i < total; ++i) { out[i].x = re[i]; out[i].y = im[i]; }
+        return CUFFT_SUCCESS;
+    }
     std::vector<double> re(total), im(total);
     for (size_t i = 0; i < total; ++i) { re[i] = in[i].x; im[i] = in[i].y; }
-    for (int axis = 0; axis < 3; ++axis) dft_axis(re, im, n, axis);
+    for (int axis = 0; axis < 3; ++axis) dft_axis<double>(re, im, n, axis);
     for (size_t i = 0; i < total; ++i) { out[i].x = (float)re[i]; out[i].y = (float)im[i]; }
     return CUFFT_SUCCESS;
 }

@@ -256,3 +256,35 @@ def test_emulated_end_to_end_tiny_poisson(tiny, impl, variant):
     assert np.all((bi == oi) | near) and np.all(np.abs(bd - od) <= DIST_TOL * od)
     hi, hd, hs = ctx.orientation_match_host(model, refs, pix, images, scale=alpha)     # the host-buffer entry point
     assert np.array_equal(hi, bi) and np.array_equal(hd, bd) and np.array_equal(hs, slices)
+
+
+def test_emulated_paper_scale_geometry_sampled(monkeypatch):
+    """Paper-scale model, fine grid (320^3) and detector (4 panels of 128 x 128, 8 x 16 lattice patches), one orientation:
+    512 blocks of each slicer on the real geometry -- every tile of the staged variant must fit and stage (no fallback) --
+    with the FFT stub in fp32 (the arithmetic cuFFT uses), 1,024 sampled points from the oracle.  At w = 8 (reading
+    s10b) the error is below 1e-6; w = 7 left 6e-6 here and up to 1.8e-5 on other samples."""
+    monkeypatch.setenv("SPF_EMU_FFT32", "1")
+    cfg = CONFIGS["paper_scale"]
+    model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(1, seed=2)
+    ctx = EmuContext(cfg.N, eps=cfg.eps)
+    assert (ctx.info.n_fine, ctx.info.w) == (320, 8)
+    ctx.set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    ctx.prepare_model(model)
+    assert ctx.info.grid_is_real == 1
+    rng = np.random.default_rng(6)
+    sj = rng.integers(0, cfg.P, 1024)
+    ref = orc.slice_points(model, refs, pix, np.zeros(1024, np.int64), sj)
+    outs = {}
+    for impl in (1, 2):
+        ctx.set_option("slice_impl", impl)
+        eb.counters()
+        outs[impl] = ctx.slice(refs, pix, SPF_OUT_COMPLEX)
+        n = eb.counters()
+        err = _rel(outs[impl][0, sj], ref)
+        print("paper-scale geometry, slice_impl %d: relative L2 %.2e, %d bulk tensor copies" % (impl, err, n["tma_copies"]))
+        assert err <= 2e-6
+        if impl == 2:
+            assert n["tma_copies"] >= 512 * 8                  # every one of the 512 blocks staged its box, >= 8 x-planes each
+    assert _rel(outs[2], outs[1]) <= 2e-6
