@@ -203,13 +203,38 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *   "match_refine": [1] = recompute the winner's distance in the difference form; 0 = return the epilogue's own value
  * The defaults are the variants with the least machinery (classic CUDA: no TMA, mbarrier or tcgen05).  The others
  * have not yet run on hardware and are opt-in: the caller switches them on once they have been
- * checked on the device at hand (the Python binding's SpfContext.spf_autotune does that in a child process,
- * DESIGN.md section 7).
+ * checked on the device at hand: spf_selftest (below) checks one and switches it on; the Python binding's
+ * SpfContext.spf_autotune runs the same call in a child process first.
+ *   "selftest_small": [0]; 1 = spf_selftest runs its small cases (a few hundred image-slice pairs): quick checks
  *   "record_events": [0]; 1 = spf_slice / spf_match record CUDA events on their stream around the
  *                    dominant kernels, read back with spf_last_kernel_ms
  * Returns SPF_EINVAL for an unknown key or value.
  */
 SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
+
+/*
+ * Device self-check of one kernel variant against this library's reference kernels, and the switch that turns a verified
+ * variant on.  variant: "slice_gcoop" (slice_impl 3), "slice_coop" (slice_impl 2), "match_cg1", "match_cg2" (the tcgen05
+ * matcher on single CTAs / CTA pairs).  Slicing variants slice the caller's own prepared model (read-only; SPF_ESTATE
+ * before spf_prepare_model) at 16 seeded orientations x 4,096 pixels with the reference gather and with the variant
+ * (bar: relative L2 <= 3e-6, all finite); matcher variants run two seeded cases, with and without a mask, against
+ * spf_match_reference (bar: distances within 1e-4 d; without the refinement 1e-4 d + 2e-6 of the norms; argmin equal
+ * outside near-ties).  A consistency check between two CUDA paths, not parity (tests/ hold every variant to the oracle).
+ * On success (report->passed = 1) the variant becomes the context's choice -- for slicers only if it was also the
+ * fastest verified so far, pairs supersede the single-CTA matcher -- so a C caller reaches the TMA / tcgen05 kernels
+ * with spf_create + spf_prepare_model + spf_selftest, no other option set.  Returns SPF_OK when the check RAN (passed or
+ * not), another status when it could not (SPF_EFAULT: the variant's watchdog gave up).  Synchronises.  Runs in the
+ * calling process: a variant that raises an SM exception takes the caller's CUDA context with it; callers that need
+ * containment run it in a child process first (the Python binding's spf_autotune does).  report [host].
+ */
+typedef struct {
+    int32_t passed;      /* 1 = the variant agrees with the reference kernels */
+    float ms_variant;    /* device time of the variant on the check's timing case (CUDA events) */
+    float ms_reference;  /* the same for the reference kernel */
+    double worst_rel;    /* slicers: relative L2 difference; matchers: worst relative distance error (refined result) */
+    char detail[192];    /* one line of text */
+} spf_selftest_report;
+SPF_API int spf_selftest(spf_ctx *ctx, const char *variant, spf_selftest_report *report, void *stream);
 
 /*
  * Watchdog.  Every wait on a hardware barrier inside the slicing and matching kernels is bounded

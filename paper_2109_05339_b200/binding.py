@@ -21,7 +21,7 @@ EXPORTS = ["spf_version", "spf_status_string", "spf_plan_kernel_width", "spf_pla
            "spf_get_info", "spf_last_error", "spf_set_detector_layout", "spf_prepare_model", "spf_slice", "spf_match",
            "spf_match_workspace_bytes", "spf_match_reference", "spf_orientation_match_host", "spf_debug_deapodisation",
            "spf_debug_fine_grid", "spf_set_option", "spf_launch_count", "spf_last_kernel_ms", "spf_last_match_products",
-           "spf_check_fault"]
+           "spf_check_fault", "spf_selftest"]
 
 
 class SpfParams(C.Structure):
@@ -32,6 +32,11 @@ class SpfParams(C.Structure):
 class SpfInfo(C.Structure):
     _fields_ = [("n", C.c_int32), ("n_fine", C.c_int32), ("w", C.c_int32), ("beta", C.c_double),
                 ("n_padded", C.c_int32), ("grid_is_real", C.c_int32), ("prepared", C.c_int32), ("sm_count", C.c_int32)]
+
+
+class SpfSelftestReport(C.Structure):
+    _fields_ = [("passed", C.c_int32), ("ms_variant", C.c_float), ("ms_reference", C.c_float), ("worst_rel", C.c_double),
+                ("detail", C.c_char * 192)]
 
 
 class SpfError(RuntimeError):
@@ -81,6 +86,7 @@ def load_library():
     lib.spf_last_kernel_ms.argtypes = [vp, i32, C.POINTER(C.c_float)]
     lib.spf_last_match_products.argtypes = [vp, C.POINTER(i32)]
     lib.spf_check_fault.argtypes = [vp, vp]
+    lib.spf_selftest.argtypes = [vp, C.c_char_p, C.POINTER(SpfSelftestReport), vp]
     _lib = lib
     return lib
 
@@ -150,6 +156,13 @@ class SpfContext:
     def spf_check_fault(self):
         """Synchronise the current stream; raise SpfError(SPF_EFAULT) if a kernel's watchdog gave up."""
         self._check(self._lib.spf_check_fault(self._h, _stream(self.device)))
+
+    def spf_selftest(self, variant: str) -> dict:
+        """The library's own in-process check of one variant (spf.h); on success the library switches it on."""
+        rep = SpfSelftestReport()
+        self._check(self._lib.spf_selftest(self._h, variant.encode(), C.byref(rep), _stream(self.device)))
+        return {"passed": bool(rep.passed), "ms_variant": float(rep.ms_variant), "ms_reference": float(rep.ms_reference),
+                "worst_rel": float(rep.worst_rel), "detail": rep.detail.decode(errors="replace")}
 
     def spf_autotune(self, timeout_s: float = 240.0) -> dict:
         """Switch on the faster kernel variants that pass the device self-check (selfcheck.py, run once per

@@ -104,6 +104,7 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     if (!strcmp(key, "match_chunk_kblocks") && value >= 0 && value <= (1 << 20)) { ctx->opt_match_chunk_kb = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_condition") && (value == 0 || value == 1)) { ctx->opt_match_condition = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_refine") && (value == 0 || value == 1)) { ctx->opt_match_refine = (int)value; return SPF_OK; }
+    if (!strcmp(key, "selftest_small") && (value == 0 || value == 1)) { ctx->opt_selftest_small = (int)value; return SPF_OK; }
     if (!strcmp(key, "record_events") && (value == 0 || value == 1)) { ctx->opt_record_events = (int)value; return SPF_OK; }
     return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
 }

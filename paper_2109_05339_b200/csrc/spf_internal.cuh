@@ -39,6 +39,8 @@ struct spf_ctx {
     int opt_match_refine = 1;                   // 1 = recompute the winner's distance in the difference form
     int gemm_max_clusters[2][2] = {{0, 0}, {0, 0}};  // [CG - 1][NI - 1]: co-resident clusters of k_match_gemm, 0 = not asked yet
     int opt_record_events = 0;
+    int opt_selftest_small = 0;                 // 1 = spf_selftest uses its small cases (quick checks, the emulator)
+    float selftest_slice_ms = 0.f;              // time of the fastest slicer spf_selftest has verified and switched on (0: none yet)
     int64_t launches = 0;
     // CUDA events around the dominant kernels (option "record_events"): [0,1] slice kernel,
     // [2,3] match GEMM, [4] start of the match operand preparation (which ends at [2])

@@ -7,12 +7,13 @@ TMA-staged shared-memory gather, one warp per point; tcgen05 GEMM on single CTAs
 hand, and among the slicing variants that pass, the one the check timed fastest.
 
 A check runs in a CHILD process (`python -m paper_2109_05339_b200.selfcheck <variant>`): a kernel
-that faults poisons its CUDA context, and the caller's must survive that.  The child compares the
-variant with another computation made by the library's own kernels on the same device -- the
-staged gather with the global gather, the tensor-core matcher with the CUDA-core difference-form
-matcher (`spf_match_reference`) -- on seeded random inputs that span several tiles and a ragged
-tail.  This is a consistency check between two CUDA paths, not parity: parity against the oracle
-is what tests/ does.  Nothing here touches `oracle/`.
+that faults poisons its CUDA context, and the caller's must survive that.  The child calls the C library's own
+check, `spf_selftest` (include/spf.h, csrc/spf_selftest.cu): the variant against another computation made by the
+library's reference kernels on the same device -- the warp-per-point gathers against the one-thread-per-point
+gather, the tensor-core matcher against the CUDA-core difference-form reference -- on seeded inputs that span
+several tiles and a ragged tail.  All comparison logic is in C; this module only provides the process boundary,
+the ordering and the verdict cache.  It is a consistency check between two CUDA paths, not parity: parity
+against the oracle is what tests/ does.  Nothing here touches `oracle/`.
 
 Exit status of the child: 0 = variant agrees, 1 = disagrees with the reference kernels or the library's
 watchdog reported SPF_EFAULT (a verdict about the kernel), 3 = the check itself could not run (import error,
@@ -39,145 +40,57 @@ _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
 
 
-def _check_slice_staged(device: int, impl: int):
+def _even_model(n: int, seed: int, even: bool):
+    """Seeded random model; `even` makes it exactly even about index floor(n/2) (real fine grid)."""
     import torch
-    from .binding import SpfContext, SPF_OUT_COMPLEX
-    dev = torch.device("cuda", device)
-    g = torch.Generator(device="cpu"); g.manual_seed(11)
-    worst = 0.0
-    for n, eps, even in ((24, 1e-6, True), (21, 1e-6, False), (20, 1e-9, True)):
-        A = torch.randn((n, n, n), generator=g, dtype=torch.float32)
-        if even:   # A[n] == A[-n] about index floor(n/2): exercises the real-grid kernels
-            c = n // 2
-            idx = (2 * c - torch.arange(n)) % n
-            Af = A[idx][:, idx][:, :, idx]
-            A = 0.5 * (A + Af)
-            if n % 2 == 0:
-                A[0] = 0; A[:, 0] = 0; A[:, :, 0] = 0
-        rows = cols = 40     # 1,600 pixels: 8 x 16 lattice patches with ragged edges
-        u = (torch.arange(cols, dtype=torch.float64) - (cols - 1) / 2) / cols
-        v = (torch.arange(rows, dtype=torch.float64) - (rows - 1) / 2) / rows
-        vv, uu = torch.meshgrid(v, u, indexing="ij")
-        k = torch.stack([uu, vv, torch.ones_like(uu)], -1)
-        q = k / k.norm(dim=-1, keepdim=True) - torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64)
-        pix = (q * (0.9 * torch.pi / q.norm(dim=-1).max())).reshape(-1, 3).to(torch.float32)
-        quats = torch.randn((37, 4), generator=g, dtype=torch.float32)
-        ctx = SpfContext(n, eps=eps, device=device)
-        ctx.spf_set_detector_layout(1, rows, cols)
-        ctx.spf_prepare_model(A.to(dev))
-        assert bool(ctx.info.grid_is_real) == even
-        outs = []
-        for which in (1, impl):
-            ctx.spf_set_option("slice_impl", which)
-            outs.append(ctx.spf_slice(quats.to(dev), pix.to(dev), SPF_OUT_COMPLEX))
-            ctx.spf_check_fault()
-        err = float((outs[1] - outs[0]).abs().pow(2).sum().sqrt() / outs[0].abs().pow(2).sum().sqrt())
-        worst = max(worst, err)
-        # the two variants differ only in how the kernel weights are evaluated (polynomial fit vs exp/sqrt)
-        if not err <= 3e-6:
-            raise AssertionError("staged vs global gather: relative L2 %.3e (n=%d eps=%g)" % (err, n, eps))
-        ctx.close()
-    return "slice_impl %d == global gather to %.1e" % (impl, worst), _time_slice(device, impl)
-
-
-def _time_slice(device: int, impl: int) -> dict:
-    """Milliseconds of spf_slice for 64 orientations x 65,536 pixels (4 panels of 128 x 128, about 0.9 fine cells
-    per pixel as at Paper-scale) of a 128^3 even model (real grid of 266^3 cells = 75 MB: beyond L1, inside L2,
-    w = 7), global gather and variant `impl`, best of 3 (CUDA events on the current stream)."""
-    import torch
-    from .binding import SpfContext, SPF_OUT_INTENSITY
-    dev = torch.device("cuda", device)
-    g = torch.Generator(device="cpu"); g.manual_seed(3)
-    n = 128
+    g = torch.Generator(device="cpu"); g.manual_seed(seed)
     A = torch.randn((n, n, n), generator=g, dtype=torch.float32)
-    idx = (2 * (n // 2) - torch.arange(n)) % n
-    A = 0.5 * (A + A[idx][:, idx][:, :, idx])
-    A[0] = 0; A[:, 0] = 0; A[:, :, 0] = 0
-    edge = 128
-    t = (torch.arange(edge, dtype=torch.float64) - (edge - 1) / 2) / (2 * edge)
-    pix = []
-    for cy in (-0.26, 0.26):
-        for cx in (-0.26, 0.26):
-            vv, uu = torch.meshgrid(t + cy, t + cx, indexing="ij")
-            k = torch.stack([uu, vv, torch.ones_like(uu)], -1)
-            pix.append((k / k.norm(dim=-1, keepdim=True) - torch.tensor([0.0, 0.0, 1.0], dtype=torch.float64)).reshape(-1, 3))
-    pix = torch.cat(pix)
-    pix = (pix * (0.9 * torch.pi / pix.norm(dim=-1).max())).to(torch.float32).to(dev)
-    n_or = 64
-    quats = torch.randn((n_or, 4), generator=g, dtype=torch.float32).to(dev)
-    ctx = SpfContext(n, eps=1e-6, device=device)
-    ctx.spf_set_detector_layout(4, edge, edge)
-    ctx.spf_prepare_model(A.to(dev))
-    out = torch.empty((n_or, pix.shape[0]), dtype=torch.float32, device=dev)
-    ms = {}
-    for which in (1, impl):
-        ctx.spf_set_option("slice_impl", which)
-        best = float("inf")
-        for rep in range(4):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            ctx.spf_slice(quats, pix, SPF_OUT_INTENSITY, out=out)
-            e1.record()
-            e1.synchronize()
-            if rep:
-                best = min(best, e0.elapsed_time(e1))
-        ctx.spf_check_fault()
-        ms["global" if which == 1 else "variant"] = best
-    ctx.close()
-    return {"slice_ms_global": ms["global"], "slice_ms": ms["variant"], "points": n_or * int(pix.shape[0])}
+    if even:
+        idx = (2 * (n // 2) - torch.arange(n)) % n
+        A = 0.5 * (A + A[idx][:, idx][:, :, idx])
+        if n % 2 == 0:
+            A[0] = 0; A[:, 0] = 0; A[:, :, 0] = 0
+    return A
 
 
-def _check_match(device: int, cta_group: int) -> str:
+def _check_slice(device: int, variant: str):
+    """The comparison itself is the C library's (spf_selftest, csrc/spf_selftest.cu): this only chooses the models
+    it is run on -- real and complex fine grid, w = 8 and w = 10, and a 128^3 model (a 266^3-cell grid: beyond L1,
+    inside L2) whose timing decides between the slicing variants."""
     import torch
     from .binding import SpfContext
     dev = torch.device("cuda", device)
-    g = torch.Generator(device="cpu"); g.manual_seed(5 + cta_group)
+    worst, metrics = 0.0, {}
+    for n, eps, even, timed in ((24, 1e-6, True, False), (21, 1e-6, False, False), (20, 1e-9, True, False), (128, 1e-6, True, True)):
+        ctx = SpfContext(n, eps=eps, device=device)
+        ctx.spf_prepare_model(_even_model(n, 11 + n, even).to(dev))
+        assert bool(ctx.info.grid_is_real) == even
+        r = ctx.spf_selftest(variant)
+        ctx.close()
+        if not r["passed"]:
+            raise AssertionError(r["detail"])
+        worst = max(worst, r["worst_rel"])
+        if timed:
+            metrics = {"slice_ms_global": r["ms_reference"], "slice_ms": r["ms_variant"]}
+    return "%s == reference gather to %.1e" % (variant, worst), metrics
+
+
+def _check_match(device: int, variant: str) -> str:
+    from .binding import SpfContext
     ctx = SpfContext(8, device=device)
-    ctx.spf_set_option("match_impl", 0)             # the tcgen05 kernel (the library default is the CUDA-core matcher)
-    ctx.spf_set_option("match_cta_group", cta_group)
-    worst = 0.0
-    for n_img, M, P, counts in ((300, 513, 2048, True), (130, 257, 200, False), (5, 40, 4100, True)):
-        S = torch.rand((M, P), generator=g) * torch.rand((M, 1), generator=g) * 3.0
-        pick = torch.randint(0, M, (n_img,), generator=g)
-        I = torch.poisson(S[pick], generator=g) if counts else S[pick] + 0.1 * torch.rand((n_img, P), generator=g)
-        mask = (torch.rand(P, generator=g) > 0.2).to(torch.uint8)
-        for mk in (None, mask):
-            dI, dS = I.to(dev).contiguous(), S.to(dev).contiguous()
-            dm = None if mk is None else mk.to(dev)
-            ri, rd, dist = ctx.spf_match_reference(dI, dS, dm)
-            keep = torch.ones(P, device=dev) if dm is None else dm.float()
-            nrm = (dI * dI * keep).sum(1) + ((dS * dS * keep).sum(1))[ri.long()]
-            for refine in (1, 0):
-                ctx.spf_set_option("match_refine", refine)
-                bi, bd = ctx.spf_match(dI, dS, dm)
-                ctx.spf_check_fault()
-                torch.cuda.synchronize(dev)
-                # refine = 1 (the library's result): 1e-4 of d against the CUDA-core difference-form reference.
-                # refine = 0 exposes the epilogue's own a_i + b_m - 2 G: a sanity bound on the contraction itself,
-                # 1e-4 d plus 2e-6 of the norms (the expansion's fp32 cancellation floor); not a parity bar.
-                tol = 1e-4 * rd if refine else 1e-4 * rd + 2e-6 * nrm
-                rel = ((bd - rd).abs() / rd.clamp_min(1e-30)).max().item()
-                if refine:
-                    worst = max(worst, rel)
-                if not bool(((bd - rd).abs() <= tol).all()):
-                    raise AssertionError("cta_group %d (refine %d): distance differs from the CUDA-core matcher by %.3e" % (cta_group, refine, rel))
-                # argmin may differ only where the reference's own margin is within tolerance
-                d_at = dist.gather(1, bi.long().clamp(0, M - 1)[:, None])[:, 0]
-                bad = (bi != ri) & ((d_at - rd) > tol)
-                if bool(bad.any()) or bool((bi < 0).any()) or bool((bi >= M).any()):
-                    raise AssertionError("cta_group %d (refine %d): argmin differs from the CUDA-core matcher" % (cta_group, refine))
+    r = ctx.spf_selftest(variant)
     ctx.close()
-    return "cta_group::%d == CUDA-core matcher, distances to %.1e" % (cta_group, worst)
+    if not r["passed"]:
+        raise AssertionError(r["detail"])
+    return r["detail"]
 
 
 def run_variant(variant: str, device: int = 0):
     """Returns (one-line description, metrics dict)."""
     if variant in SLICE_IMPL:
-        return _check_slice_staged(device, SLICE_IMPL[variant])
-    if variant == "match_cg1":
-        return _check_match(device, 1), {}
-    if variant == "match_cg2":
-        return _check_match(device, 2), {}
+        return _check_slice(device, variant)
+    if variant in ("match_cg1", "match_cg2"):
+        return _check_match(device, variant), {}
     raise ValueError("unknown variant %r (one of %s)" % (variant, ", ".join(VARIANTS)))
 
 

@@ -24,6 +24,11 @@ class SpfInfo(C.Structure):
                 ("n_padded", C.c_int32), ("grid_is_real", C.c_int32), ("prepared", C.c_int32), ("sm_count", C.c_int32)]
 
 
+class SelftestReport(C.Structure):
+    _fields_ = [("passed", C.c_int32), ("ms_variant", C.c_float), ("ms_reference", C.c_float), ("worst_rel", C.c_double),
+                ("detail", C.c_char * 192)]
+
+
 class EmuError(RuntimeError):
     def __init__(self, status, text):
         super().__init__("libspf (emulated) status %d: %s" % (status, text))
@@ -55,6 +60,7 @@ def lib():
         L.spf_debug_fine_grid.argtypes = [vp, vp, vp]
         L.spf_debug_deapodisation.argtypes = [vp, vp]
         L.spf_launch_count.argtypes = [vp]; L.spf_launch_count.restype = i64
+        L.spf_selftest.argtypes = [vp, C.c_char_p, C.POINTER(SelftestReport), vp]
         L.spf_emu_last_fault.restype = C.c_char_p
         L.spf_emu_set_sm_count.argtypes = [C.c_int]
         L.spf_emu_counters.argtypes = [C.c_void_p, C.c_int]
@@ -109,6 +115,11 @@ class EmuContext:
 
     def set_detector_layout(self, panels, rows, cols):
         self._check(self.L.spf_set_detector_layout(self.h, panels, rows, cols))
+
+    def selftest(self, variant):
+        rep = SelftestReport()
+        self._check(self.L.spf_selftest(self.h, variant.encode(), C.byref(rep), None))
+        return {"passed": bool(rep.passed), "worst_rel": float(rep.worst_rel), "detail": rep.detail.decode(errors="replace")}
 
     def check_fault(self):
         self._check(self.L.spf_check_fault(self.h, None))

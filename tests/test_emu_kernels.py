@@ -288,3 +288,31 @@ def test_emulated_paper_scale_geometry_sampled(monkeypatch):
         if impl == 2:
             assert n["tma_copies"] >= 512 * 8                  # every one of the 512 blocks staged its box, >= 8 x-planes each
     assert _rel(outs[2], outs[1]) <= 2e-6
+
+
+def test_emulated_spf_selftest_checks_and_switches_variants_on(tiny):
+    """spf_selftest (the C library's own variant check) executed under the emulator: every variant
+    agrees with the reference kernels on the check's seeded cases, a passing matcher becomes the context's choice
+    (pairs supersede single CTAs), and a C caller needs no other option to reach the TMA / tcgen05 kernels."""
+    cfg, model, pix, refs, c_ref = tiny
+    ctx = EmuContext(cfg.N, eps=cfg.eps, sm_count=4)
+    ctx.set_option("selftest_small", 1)
+    with pytest.raises(EmuError) as e:
+        ctx.selftest("slice_coop")
+    assert e.value.status == -4                       # slicers check the caller's own model: SPF_ESTATE before prepare
+    ctx.prepare_model(model)
+    for v in ("slice_gcoop", "slice_coop", "match_cg1", "match_cg2"):
+        r = ctx.selftest(v)
+        print(v, r)
+        assert r["passed"], r
+        assert r["worst_rel"] <= (3e-6 if v.startswith("slice") else 1e-4)
+    with pytest.raises(EmuError):
+        ctx.selftest("no_such_variant")
+    # the matcher is now the tcgen05 pair kernel with no option set by the caller: MMAs are issued
+    rng = np.random.default_rng(2)
+    S = rng.random((70, 256)).astype(np.float32)
+    I = rng.poisson(S[:9]).astype(np.float32)
+    eb.counters()
+    bi, bd, prods = ctx.match(I, S)
+    assert prods == 2 and eb.counters()["mmas"] > 0
+    _check_match(bi, bd, I, S)
