@@ -154,6 +154,22 @@ SPF_API int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const fl
 SPF_API size_t spf_match_workspace_bytes(int64_t n_img, int64_t M, int64_t P);
 
 /*
+ * Steps a3-a8 fused at the a5 / a7 seam: the M orientations are sliced chunk_M at a time into a
+ * buffer inside the workspace and each chunk is matched at once, the running (distance, index) keys merging across
+ * chunks -- the [M][P] slice array never exists (26 GB at Matching-heavy; 79 GB for the paper's 1.2 M orientations x
+ * 16,384 pixels).  Same result as spf_slice into an [M][P] array followed by spf_match, with one
+ * difference on the tensor-core path: the common vector c of the conditioned expansion is the mean of the FIRST chunk's
+ * slices (any c gives the same distances in exact arithmetic), and the winners are sliced once more (n_img x P points)
+ * for the difference-form refinement of best_dist.  quats [dev] [M][4], pix_q [dev] [P][3], images [dev] [n_img][P],
+ * mask [dev] [P] or NULL, best_idx / best_dist [dev] [n_img], workspace [dev] >= spf_slice_match_workspace_bytes(n_img,
+ * min(chunk_M, M), P) bytes, 1024-byte aligned.  SPF_ESTATE before spf_prepare_model.
+ */
+SPF_API int spf_slice_match(spf_ctx *ctx, const float *quats, int64_t M, const float *pix_q, int64_t P, float scale,
+                            const float *images, int64_t n_img, const uint8_t *mask, int64_t chunk_M, int32_t *best_idx,
+                            float *best_dist, void *workspace, size_t workspace_bytes, void *stream);
+SPF_API size_t spf_slice_match_workspace_bytes(int64_t n_img, int64_t chunk_M, int64_t P);
+
+/*
  * Debug variant of spf_match for tests: additionally writes the full distance matrix
  * dist [dev] [n_img][M] fp32 with a plain CUDA-core kernel (one block per pair, difference form
  * accumulated in fp64, rounded once) -- used to check the matchers from a second, independent

@@ -21,7 +21,7 @@ EXPORTS = ["spf_version", "spf_status_string", "spf_plan_kernel_width", "spf_pla
            "spf_get_info", "spf_last_error", "spf_set_detector_layout", "spf_prepare_model", "spf_slice", "spf_match",
            "spf_match_workspace_bytes", "spf_match_reference", "spf_orientation_match_host", "spf_debug_deapodisation",
            "spf_debug_fine_grid", "spf_set_option", "spf_launch_count", "spf_last_kernel_ms", "spf_last_match_products",
-           "spf_check_fault", "spf_selftest"]
+           "spf_check_fault", "spf_selftest", "spf_slice_match", "spf_slice_match_workspace_bytes"]
 
 
 class SpfParams(C.Structure):
@@ -87,6 +87,9 @@ def load_library():
     lib.spf_last_match_products.argtypes = [vp, C.POINTER(i32)]
     lib.spf_check_fault.argtypes = [vp, vp]
     lib.spf_selftest.argtypes = [vp, C.c_char_p, C.POINTER(SpfSelftestReport), vp]
+    lib.spf_slice_match.argtypes = [vp, vp, i64, vp, i64, f32, vp, i64, vp, i64, vp, vp, vp, sz, vp]
+    lib.spf_slice_match_workspace_bytes.argtypes = [i64, i64, i64]
+    lib.spf_slice_match_workspace_bytes.restype = sz
     _lib = lib
     return lib
 
@@ -233,6 +236,27 @@ class SpfContext:
         self._check(self._lib.spf_match(self._h, _dev(images, torch.float32, "images"), n_img, _dev(slices, torch.float32, "slices"),
                                         M, P, mk, _dev(best_idx, torch.int32, "best_idx"), _dev(best_dist, torch.float32, "best_dist"),
                                         C.c_void_p(ws_ptr), need, _stream(self.device)))
+        return best_idx, best_dist
+
+    def spf_slice_match(self, quats: torch.Tensor, pix_q: torch.Tensor, images: torch.Tensor, scale: float = 1.0,
+                        mask: torch.Tensor = None, chunk_M: int = 1024):
+        """Slicing and matching fused at the seam: slices exist only chunk_M orientations at a time (spf.h)."""
+        M, P, n_img = quats.shape[0], pix_q.shape[0], images.shape[0]
+        if quats.shape != (M, 4) or pix_q.shape != (P, 3) or images.shape != (n_img, P):
+            raise ValueError("quats [M,4], pix_q [P,3], images [n_img,P]")
+        chunk_M = max(1, min(int(chunk_M), M))
+        need = int(self._lib.spf_slice_match_workspace_bytes(n_img, chunk_M, P))
+        if self._ws is None or self._ws.numel() < need + 1024:
+            self._ws = None
+            self._ws = torch.empty(need + 1024, dtype=torch.uint8, device=self.device)
+        ws_ptr = (self._ws.data_ptr() + 1023) & ~1023
+        best_idx = torch.empty(n_img, dtype=torch.int32, device=self.device)
+        best_dist = torch.empty(n_img, dtype=torch.float32, device=self.device)
+        mk = None if mask is None else _dev(mask, torch.uint8, "mask")
+        self._check(self._lib.spf_slice_match(self._h, _dev(quats, torch.float32, "quats"), M, _dev(pix_q, torch.float32, "pix_q"), P,
+                                              float(scale), _dev(images, torch.float32, "images"), n_img, mk, chunk_M,
+                                              _dev(best_idx, torch.int32, "best_idx"), _dev(best_dist, torch.float32, "best_dist"),
+                                              C.c_void_p(ws_ptr), need, _stream(self.device)))
         return best_idx, best_dist
 
     def spf_match_reference(self, images: torch.Tensor, slices: torch.Tensor, mask: torch.Tensor = None):

@@ -55,6 +55,7 @@ struct MatchArgs {
     int kblocks;            // P_pad / 64
     int chunk_kb;           // K blocks accumulated in TMEM between two drains by the epilogue (>= 1)
     int n_ib, n_mb;         // tiles along images / slices
+    uint32_t m_base;        // orientation index of slice row 0 (streaming: slices arrive in chunks of M)
     unsigned long long *keys;
     const double *aI, *bS;  // a_i = ||I_i - c||^2, b_m = sum S'_m (S'_m + 2 c)
     const uint32_t *scal;   // [2] = image plane 2 needed, [4] = eI, [5] = eS
@@ -184,10 +185,14 @@ __global__ void k_match_finalize(const unsigned long long *__restrict__ keys, in
 // cancellation.  Rows with no winner (index -1) keep their NaN.
 __global__ void __launch_bounds__(256) k_match_refine(const float *__restrict__ images, const float *__restrict__ slices,
                                                       int64_t M, int64_t P, const uint8_t *__restrict__ mask,
-                                                      const int32_t *__restrict__ best_idx, float *__restrict__ best_dist) {
+                                                      const int32_t *__restrict__ best_idx, float *__restrict__ best_dist,
+                                                      int rows_are_winners) {
+    // rows_are_winners = 0: slices is the whole [M][P] array, the winner's row is best_idx[i];
+    //                  = 1: slices holds, in row i, the slice of image i's winning orientation (streaming: re-sliced)
     const int64_t i = blockIdx.x;
-    const int64_t m = best_idx[i];
-    if (m < 0 || m >= M) return;
+    const int64_t w = best_idx[i];
+    if (w < 0 || (!rows_are_winners && w >= M)) return;
+    const int64_t m = rows_are_winners ? i : w;
     const float *I = images + i * P, *S = slices + m * P;
     double acc = 0.0;
     for (int64_t j = threadIdx.x; j < P; j += blockDim.x) {
@@ -395,7 +400,7 @@ k_match_gemm(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ 
                 for (int k = 0; k < EPI_COLS; ++k) {
                     if (m0 + k < a.M) {
                         const float d = spfmm::distance(aIv, __ldg(a.bS + m0 + k), neg2sc, acc[k]);
-                        if (d < best) { best = d; bm = (uint32_t)(m0 + k); }   // ascending k: the lowest index wins ties
+                        if (d < best) { best = d; bm = a.m_base + (uint32_t)(m0 + k); }   // ascending k: the lowest index wins ties
                     }
                 }
                 if (bm != 0xffffffffu) atomicMin(&a.keys[i], spfmm::pack_key(best, bm));
@@ -426,7 +431,7 @@ constexpr int ST_BM = 128, ST_BN = 128, ST_BK = 16, ST_PAD = 4, ST_FLUSH = 1024 
 
 __global__ void __launch_bounds__(256, 1)
 k_match_simt(const float *__restrict__ images, int64_t n_img, const float *__restrict__ slices, int64_t M, int64_t P,
-             const uint8_t *__restrict__ mask, unsigned long long *__restrict__ keys) {
+             const uint8_t *__restrict__ mask, unsigned long long *__restrict__ keys, uint32_t m_base) {
     __shared__ __align__(16) float sI[ST_BK][ST_BM + ST_PAD];
     __shared__ __align__(16) float sS[ST_BK][ST_BN + ST_PAD];
     const int tid = threadIdx.x;
@@ -490,7 +495,7 @@ k_match_simt(const float *__restrict__ images, int64_t n_img, const float *__res
         for (int v = 0; v < 8; ++v) {
             const int64_t m = m0 + (v < 4 ? tx * 4 + v : 64 + tx * 4 + v - 4);   // ascending in v: the lowest index wins ties
             const float d = tot[u][v] + acc[u][v];
-            if (m < M && d < best) { best = d; bm = (uint32_t)m; }
+            if (m < M && d < best) { best = d; bm = m_base + (uint32_t)m; }
         }
         if (i < n_img && bm != 0xffffffffu) atomicMin(&keys[i], spfmm::pack_key(best, bm));
     }
@@ -589,20 +594,11 @@ size_t spf_match_workspace_bytes(int64_t n_img, int64_t M, int64_t P) {
     return ws_layout(n_img, M, P).total;
 }
 
-int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P,
-              const uint8_t *mask, int32_t *best_idx, float *best_dist, void *workspace, size_t workspace_bytes,
-              void *stream_) {
-    if (!ctx) return SPF_EINVAL;
-    if (n_img < 0 || M < 0 || P < 0) return spf_set_err(ctx, SPF_EINVAL, "spf_match: negative size");
-    if (n_img == 0) return SPF_OK;
-    if (M < 1 || P < 1) return spf_set_err(ctx, SPF_EINVAL, "spf_match: M and P must be >= 1 when n_img >= 1");
-    if (!images || !slices || !best_idx || !best_dist || !workspace) return spf_set_err(ctx, SPF_EINVAL, "spf_match: null pointer");
-    if (M > 0x7fffffffLL || n_img > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: more than 2^31-1 rows");
-    const WsLayout L = ws_layout(n_img, M, P);
-    if (workspace_bytes < L.total) return spf_set_err(ctx, SPF_EINVAL, "spf_match: workspace %zu < required %zu bytes", workspace_bytes, L.total);
-    if (((uintptr_t)workspace & 1023u) != 0) return spf_set_err(ctx, SPF_EINVAL, "spf_match: workspace must be 1024-byte aligned");
-    cudaStream_t st = (cudaStream_t)stream_;
-    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+// One pass of the matcher over a chunk of M slices whose first row is orientation m_base.  first: reset the argmin keys,
+// (tensor-core path) take the common vector from THIS chunk and prepare the image operand; later chunks reuse both.
+// The keys merge across chunks through the same packed atomicMin, so the result is that of one pass over all slices.
+static int match_pass(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P, const uint8_t *mask,
+                      void *workspace, const WsLayout &L, cudaStream_t st, int64_t m_base, bool first) {
     uint8_t *ws = (uint8_t *)workspace;
     uint32_t *scal = (uint32_t *)(ws + L.scal);
     unsigned long long *keys = (unsigned long long *)(ws + L.keys);
@@ -612,33 +608,34 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
 
     int rc;
     if ((rc = spf_record_event(ctx, 4, st))) return rc;
-    SPF_CUDA(ctx, cudaMemsetAsync(scal, 0, 64, st));
+    if (first) SPF_CUDA(ctx, cudaMemsetAsync(scal, 0, 64, st));
+    else SPF_CUDA(ctx, cudaMemsetAsync(scal + 1, 0, 4, st));   // the slices' abs-max is per chunk
     ctx->last_match_impl = ctx->opt_match_impl;
     if (ctx->opt_match_impl == 1) {
         // CUDA-core matcher: no operand preparation, only the argmin keys are reset (all ones = "nothing seen")
         const int64_t gy = (M + ST_BN - 1) / ST_BN;
         if (gy > 65535) return spf_set_err(ctx, SPF_EINVAL, "spf_match: M too large for the CUDA-core matcher (%lld slices)", (long long)M);
-        SPF_CUDA(ctx, cudaMemsetAsync(keys, 0xff, (size_t)n_img * 8, st));
+        if (first) SPF_CUDA(ctx, cudaMemsetAsync(keys, 0xff, (size_t)n_img * 8, st));
         if ((rc = spf_record_event(ctx, 2, st))) return rc;
-        k_match_simt<<<dim3((unsigned)((n_img + ST_BM - 1) / ST_BM), (unsigned)gy), 256, 0, st>>>(images, n_img, slices, M, P, mask, keys);
+        k_match_simt<<<dim3((unsigned)((n_img + ST_BM - 1) / ST_BM), (unsigned)gy), 256, 0, st>>>(images, n_img, slices, M, P, mask, keys, (uint32_t)m_base);
         SPF_LAUNCH_CHECK(ctx);
         if ((rc = spf_record_event(ctx, 3, st))) return rc;
         ctx->last_scal = scal; ctx->last_match_stream = st;
         ctx->ev_valid[1] = ctx->ev_valid[2] = ctx->opt_record_events != 0;
-        k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
-        SPF_LAUNCH_CHECK(ctx);
         return SPF_OK;
     }
     // a6: common vector, abs-max of both operands (images raw, slices minus c), two-term fp16 split, a_i and b_m
-    SPF_CUDA(ctx, cudaMemsetAsync(cvec, 0, (size_t)L.Ppad * 4, st));
-    k_common_vector<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(slices, M, P, mask, ctx->opt_match_condition, cvec);
-    SPF_LAUNCH_CHECK(ctx);
     const int rb = ctx->sm_count * 8;
-    k_absmax<<<(unsigned)(n_img < rb ? n_img : rb), 256, 0, st>>>(images, n_img, P, mask, cvec, 0, scal + 0);
-    SPF_LAUNCH_CHECK(ctx);
+    if (first) {
+        SPF_CUDA(ctx, cudaMemsetAsync(cvec, 0, (size_t)L.Ppad * 4, st));
+        k_common_vector<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(slices, M, P, mask, ctx->opt_match_condition, cvec);
+        SPF_LAUNCH_CHECK(ctx);
+        k_absmax<<<(unsigned)(n_img < rb ? n_img : rb), 256, 0, st>>>(images, n_img, P, mask, cvec, 0, scal + 0);
+        SPF_LAUNCH_CHECK(ctx);
+        k_split<<<(unsigned)n_img, 256, 0, st>>>(images, P, L.Ppad, mask, cvec, scal, 0, n_img, plI, aI, keys);
+        SPF_LAUNCH_CHECK(ctx);
+    }
     k_absmax<<<(unsigned)(M < rb ? M : rb), 256, 0, st>>>(slices, M, P, mask, cvec, 1, scal + 1);
-    SPF_LAUNCH_CHECK(ctx);
-    k_split<<<(unsigned)n_img, 256, 0, st>>>(images, P, L.Ppad, mask, cvec, scal, 0, n_img, plI, aI, keys);
     SPF_LAUNCH_CHECK(ctx);
     k_split<<<(unsigned)M, 256, 0, st>>>(slices, P, L.Ppad, mask, cvec, scal, 1, M, plS, bS, nullptr);
     SPF_LAUNCH_CHECK(ctx);
@@ -653,6 +650,7 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     args.n_img = n_img; args.M = M; args.kblocks = (int)(L.Ppad / BK);
     args.n_ib = (int)((n_img + TILE_ROWS * CG - 1) / (TILE_ROWS * CG));
     args.n_mb = (int)((M + BN - 1) / BN);
+    args.m_base = (uint32_t)m_base;
     args.chunk_kb = ctx->opt_match_chunk_kb > 0 ? ctx->opt_match_chunk_kb : args.kblocks;   // 0 = the whole of K in TMEM
     args.keys = keys; args.aI = aI; args.bS = bS; args.scal = scal; args.fault = ctx->d_fault; args.abort_flag = ctx->d_abort;
     if ((int64_t)args.n_ib * args.n_mb > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: too many tiles");
@@ -667,11 +665,104 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     if ((rc = spf_record_event(ctx, 3, st))) return rc;
     ctx->last_scal = scal; ctx->last_match_stream = st;
     ctx->ev_valid[1] = ctx->ev_valid[2] = ctx->opt_record_events != 0;
+    return SPF_OK;
+}
+
+static int check_match_args(spf_ctx *ctx, const char *who, const void *images, int64_t n_img, int64_t M, int64_t P, const void *bi,
+                            const void *bd, const void *workspace) {
+    if (n_img < 0 || M < 0 || P < 0) return spf_set_err(ctx, SPF_EINVAL, "%s: negative size", who);
+    if (n_img == 0) return SPF_OK;
+    if (M < 1 || P < 1) return spf_set_err(ctx, SPF_EINVAL, "%s: M and P must be >= 1 when n_img >= 1", who);
+    if (!images || !bi || !bd || !workspace) return spf_set_err(ctx, SPF_EINVAL, "%s: null pointer", who);
+    if (M > 0x7fffffffLL || n_img > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "%s: more than 2^31-1 rows", who);
+    if (((uintptr_t)workspace & 1023u) != 0) return spf_set_err(ctx, SPF_EINVAL, "%s: workspace must be 1024-byte aligned", who);
+    return SPF_OK;
+}
+
+int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *slices, int64_t M, int64_t P,
+              const uint8_t *mask, int32_t *best_idx, float *best_dist, void *workspace, size_t workspace_bytes,
+              void *stream_) {
+    if (!ctx) return SPF_EINVAL;
+    int rc = check_match_args(ctx, "spf_match", images, n_img, M, P, best_idx, best_dist, workspace);
+    if (rc || n_img == 0) return rc;
+    if (!slices) return spf_set_err(ctx, SPF_EINVAL, "spf_match: null pointer");
+    const WsLayout L = ws_layout(n_img, M, P);
+    if (workspace_bytes < L.total) return spf_set_err(ctx, SPF_EINVAL, "spf_match: workspace %zu < required %zu bytes", workspace_bytes, L.total);
+    cudaStream_t st = (cudaStream_t)stream_;
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    if ((rc = match_pass(ctx, images, n_img, slices, M, P, mask, workspace, L, st, 0, true))) return rc;
+    unsigned long long *keys = (unsigned long long *)((uint8_t *)workspace + L.keys);
     k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
     SPF_LAUNCH_CHECK(ctx);
-    if (ctx->opt_match_refine) {
-        k_match_refine<<<(unsigned)n_img, 256, 0, st>>>(images, slices, M, P, mask, best_idx, best_dist);
+    if (ctx->opt_match_impl == 0 && ctx->opt_match_refine) {
+        k_match_refine<<<(unsigned)n_img, 256, 0, st>>>(images, slices, M, P, mask, best_idx, best_dist, 0);
         SPF_LAUNCH_CHECK(ctx);
+    }
+    return SPF_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// slices produced in chunks of chunk_M orientations and consumed by the matcher at once,
+// so the [M][P] slice array never exists (26 GB at Matching-heavy, 79 GB for the paper-shaped workload)
+// ------------------------------------------------------------------------------------------
+__global__ void k_gather_quats(const float *__restrict__ quats, const int32_t *__restrict__ best_idx, int64_t n, int64_t M,
+                               float *__restrict__ out) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int64_t m = best_idx[i];
+    if (m < 0 || m >= M) m = 0;   // no winner: any valid orientation (k_match_refine skips the row)
+    for (int c = 0; c < 4; ++c) out[4 * i + c] = quats[4 * m + c];
+}
+
+struct StreamLayout { WsLayout match; size_t chunk_slices, quats, total; };
+static StreamLayout stream_layout(int64_t n_img, int64_t chunk_M, int64_t P) {
+    StreamLayout S{};
+    S.match = ws_layout(n_img, chunk_M, P);
+    size_t off = S.match.total;
+    S.chunk_slices = off; off += rup((size_t)chunk_M * P * 4, 1024);
+    S.quats = off; off += rup((size_t)chunk_M * 16, 1024);
+    S.total = off;
+    return S;
+}
+
+size_t spf_slice_match_workspace_bytes(int64_t n_img, int64_t chunk_M, int64_t P) {
+    if (n_img < 0 || chunk_M < 1 || P < 0) return 0;
+    return stream_layout(n_img, chunk_M, P).total;
+}
+
+int spf_slice_match(spf_ctx *ctx, const float *quats, int64_t M, const float *pix_q, int64_t P, float scale, const float *images,
+                    int64_t n_img, const uint8_t *mask, int64_t chunk_M, int32_t *best_idx, float *best_dist, void *workspace,
+                    size_t workspace_bytes, void *stream_) {
+    if (!ctx) return SPF_EINVAL;
+    int rc = check_match_args(ctx, "spf_slice_match", images, n_img, M, P, best_idx, best_dist, workspace);
+    if (rc || n_img == 0) return rc;
+    if (!quats || !pix_q) return spf_set_err(ctx, SPF_EINVAL, "spf_slice_match: null pointer");
+    if (chunk_M < 1) return spf_set_err(ctx, SPF_EINVAL, "spf_slice_match: chunk_M must be >= 1");
+    if (chunk_M > M) chunk_M = M;
+    const StreamLayout S = stream_layout(n_img, chunk_M, P);
+    if (workspace_bytes < S.total) return spf_set_err(ctx, SPF_EINVAL, "spf_slice_match: workspace %zu < required %zu bytes", workspace_bytes, S.total);
+    cudaStream_t st = (cudaStream_t)stream_;
+    SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
+    uint8_t *ws = (uint8_t *)workspace;
+    float *chunk = (float *)(ws + S.chunk_slices), *wq = (float *)(ws + S.quats);
+    for (int64_t m0 = 0; m0 < M; m0 += chunk_M) {
+        const int64_t Mc = M - m0 < chunk_M ? M - m0 : chunk_M;
+        if ((rc = spf_slice(ctx, quats + 4 * m0, Mc, pix_q, P, SPF_OUT_INTENSITY, scale, chunk, st))) return rc;
+        if ((rc = match_pass(ctx, images, n_img, chunk, Mc, P, mask, workspace, S.match, st, m0, m0 == 0))) return rc;
+    }
+    unsigned long long *keys = (unsigned long long *)(ws + S.match.keys);
+    k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
+    SPF_LAUNCH_CHECK(ctx);
+    if (ctx->opt_match_impl == 0 && ctx->opt_match_refine) {
+        // the winners' slices no longer exist: slice them again, chunk_M images at a time (n_img x P points in all)
+        for (int64_t i0 = 0; i0 < n_img; i0 += chunk_M) {
+            const int64_t nc = n_img - i0 < chunk_M ? n_img - i0 : chunk_M;
+            k_gather_quats<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(quats, best_idx + i0, nc, M, wq);
+            SPF_LAUNCH_CHECK(ctx);
+            if ((rc = spf_slice(ctx, wq, nc, pix_q, P, SPF_OUT_INTENSITY, scale, chunk, st))) return rc;
+            k_match_refine<<<(unsigned)nc, 256, 0, st>>>(images + i0 * P, chunk, nc, P, mask, best_idx + i0, best_dist + i0, 1);
+            SPF_LAUNCH_CHECK(ctx);
+        }
     }
     return SPF_OK;
 }

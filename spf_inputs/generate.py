@@ -39,6 +39,10 @@ CONFIGS = {
     "paper_scale": Config("paper_scale", 151, 2000, 50.0, 4, 128, 10_000, 10_000, 1e4, 1e-6, 0.05),
     "matching_heavy": Config("matching_heavy", 151, 2000, 50.0, 4, 128, 100_000, 20_000, 1e4, 1e-6, 0.05),
     "slicing_heavy": Config("slicing_heavy", 201, 5000, 70.0, 4, 128, 20_000, 2_000, 1e4, 1e-9),
+    # the paper's own per-node workload: 128 x 128-pixel images, 1,000 images
+    # against 1,200,000 model orientations.  The model size is not stated; the Paper-scale model is reused.  The slice
+    # array would be 79 GB, so this configuration runs through spf_slice_match (slices exist one chunk at a time).
+    "paper_shaped": Config("paper_shaped", 151, 2000, 50.0, 1, 128, 1_200_000, 1_000, 1e4, 1e-6, 0.05),
 }
 
 

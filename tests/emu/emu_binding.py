@@ -60,6 +60,8 @@ def lib():
         L.spf_debug_fine_grid.argtypes = [vp, vp, vp]
         L.spf_debug_deapodisation.argtypes = [vp, vp]
         L.spf_launch_count.argtypes = [vp]; L.spf_launch_count.restype = i64
+        L.spf_slice_match.argtypes = [vp, vp, i64, vp, i64, f32, vp, i64, vp, i64, vp, vp, vp, sz, vp]
+        L.spf_slice_match_workspace_bytes.argtypes = [i64, i64, i64]; L.spf_slice_match_workspace_bytes.restype = sz
         L.spf_selftest.argtypes = [vp, C.c_char_p, C.POINTER(SelftestReport), vp]
         L.spf_emu_last_fault.restype = C.c_char_p
         L.spf_emu_set_sm_count.argtypes = [C.c_int]
@@ -161,6 +163,19 @@ class EmuContext:
         prods = C.c_int32()
         self._check(self.L.spf_last_match_products(self.h, C.byref(prods)))
         return bi, bd, int(prods.value)
+
+    def slice_match(self, quats, pix, images, scale=1.0, mask=None, chunk_M=16):
+        quats, pix, images = (np.ascontiguousarray(a, np.float32) for a in (quats, pix, images))
+        M, P, n_img = quats.shape[0], pix.shape[0], images.shape[0]
+        need = self.L.spf_slice_match_workspace_bytes(n_img, min(chunk_M, M), P)
+        ws = np.full(need + 1024, 0xFF, np.uint8)
+        wp = (ws.ctypes.data + 1023) & ~1023
+        bi, bd = np.full(n_img, -7, np.int32), np.full(n_img, np.nan, np.float32)
+        mk = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+        self._check(self.L.spf_slice_match(self.h, _p(quats), M, _p(pix), P, float(scale), _p(images), n_img, _p(mk), chunk_M,
+                                           _p(bi), _p(bd), C.c_void_p(wp), need, None))
+        self.check_fault()
+        return bi, bd
 
     def match_reference(self, images, slices, mask=None):
         images, slices = np.ascontiguousarray(images, np.float32), np.ascontiguousarray(slices, np.float32)

@@ -316,3 +316,29 @@ def test_emulated_spf_selftest_checks_and_switches_variants_on(tiny):
     bi, bd, prods = ctx.match(I, S)
     assert prods == 2 and eb.counters()["mmas"] > 0
     _check_match(bi, bd, I, S)
+
+
+@pytest.mark.parametrize("impl,variant", [(1, "simt"), (2, "cg1"), (2, "cg2")])
+def test_emulated_streaming_slice_match_equals_the_two_step_path(tiny, impl, variant):
+    """spf_slice_match: 64 orientations in ragged chunks of 24 -- the slice array never exists -- give
+    the argmin and distances of spf_slice + spf_match, and agree with the oracle end to end."""
+    cfg, model, pix, refs, c_ref = tiny
+    truth, _ = planted_truth_quaternions(cfg.n_img, refs)
+    alpha = photon_scale(c_ref.real, None, cfg.photons)
+    images = poisson_images(alpha * orc.slice_points(model, truth, pix).real)
+    mask = (np.random.default_rng(1).random(cfg.P) > 0.05).astype(np.uint8)
+    ctx = EmuContext(cfg.N, eps=cfg.eps)
+    ctx.set_detector_layout(1, 32, 32)
+    ctx.set_option("slice_impl", impl)
+    _matcher(ctx, variant)
+    ctx.prepare_model(model)
+    slices = ctx.slice(refs, pix, SPF_OUT_INTENSITY, scale=alpha)
+    bi2, bd2, _ = ctx.match(images, slices, mask)
+    bi, bd = ctx.slice_match(refs, pix, images, scale=alpha, mask=mask, chunk_M=24)
+    assert np.array_equal(bi, bi2)
+    assert np.allclose(bd, bd2, rtol=(0 if variant == "simt" else 1e-6), atol=0)
+    oi, od, osd, _ = orc.match(images, alpha * c_ref.real, mask)
+    near = (osd - od) <= DIST_TOL * od
+    assert np.all((bi == oi) | near) and np.all(np.abs(bd - od) <= DIST_TOL * od)
+    one, _ = ctx.slice_match(refs, pix, images, scale=alpha, mask=mask, chunk_M=1000)     # chunk_M > M: a single chunk
+    assert np.array_equal(one, bi)

@@ -97,3 +97,66 @@ def test_matching_heavy_sampled(spf):
     assert int(bi.min()) >= 0 and int(bi.max()) < cfg.M and bool(torch.isfinite(bd).all())
     print("matching-heavy: 8 sampled rows agree with the oracle (%d near-ties), %d images matched their truth slice"
           % (int(near.sum()), int((bi.long() == truth).sum())))
+
+
+def test_streaming_equals_two_step_on_small(spf):
+    """spf_slice_match on Small: 1,024 orientations in ragged chunks of 300 give the argmin and the
+    distances of spf_slice into an [M][P] array followed by spf_match."""
+    cfg = CONFIGS["small"]
+    model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    refs = random_quaternions(cfg.M, seed=2)
+    ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+    ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    print("streaming (small) runs with", choose_variants(ctx))
+    ctx.spf_prepare_model(_dev(model))
+    d_refs, d_pix = _dev(refs), _dev(pix)
+    slices = ctx.spf_slice(d_refs, d_pix, spf.SPF_OUT_INTENSITY, scale=1.0)
+    alpha = photon_scale(slices, None, cfg.photons)
+    slices *= alpha
+    g = torch.Generator(device="cuda"); g.manual_seed(3)
+    truth = torch.randint(0, cfg.M, (256,), generator=g, device="cuda")
+    images = poisson_images(slices[truth], seed=4)
+    bi2, bd2 = ctx.spf_match(images, ctx.spf_slice(d_refs, d_pix, spf.SPF_OUT_INTENSITY, scale=alpha))
+    bi, bd = ctx.spf_slice_match(d_refs, d_pix, images, scale=alpha, chunk_M=300)
+    ctx.spf_check_fault()
+    assert torch.equal(bi, bi2) and torch.allclose(bd, bd2, rtol=1e-6, atol=0)
+
+
+def test_paper_shaped_streaming_sampled(spf):
+    """The paper's per-node workload: 1,000 images of 128 x 128 pixels against
+    1,200,000 orientations, 2e13 pixel pairs, slices alive 8,192 orientations at a time (the full array would be 79 GB).
+    The oracle cannot slice 2e10 points, so the check is by properties that hold at any size: (1) images drawn from
+    reference orientation k at high photon count must come back as k; (2) for 32 sampled images the streaming winner
+    must be the argmin, with the same distance, of the ORACLE's brute force over a subset of 2,048 orientations that
+    contains it, on slices from the (parity-tested) two-step path."""
+    cfg = CONFIGS["paper_shaped"]
+    if _free_gb() < 20:
+        pytest.skip("needs 20 GB of free device memory")
+    model = make_model(cfg.N, cfg.n_atoms, cfg.atom_radius)
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    mask = make_mask(cfg.panels, cfg.panel_edge, cfg.masked_frac)
+    refs = random_quaternions(cfg.M, seed=2)
+    ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+    ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
+    print("paper-shaped runs with", choose_variants(ctx))
+    ctx.spf_prepare_model(_dev(model))
+    d_refs, d_pix, d_mask = _dev(refs), _dev(pix), _dev(mask)
+    rng = np.random.default_rng(7)
+    planted = rng.integers(0, cfg.M, cfg.n_img)
+    lam = ctx.spf_slice(_dev(refs[planted]), d_pix, spf.SPF_OUT_INTENSITY, scale=1.0)
+    alpha = photon_scale(lam, mask, 1e5)                       # bright enough that the planted orientation wins
+    images = poisson_images(lam * alpha, seed=4)
+    bi, bd = ctx.spf_slice_match(d_refs, d_pix, images, scale=alpha, mask=d_mask, chunk_M=8192)
+    ctx.spf_check_fault()
+    bi_h, bd_h = bi.cpu().numpy(), bd.cpu().numpy()
+    assert int(bi.min()) >= 0 and int(bi.max()) < cfg.M and np.isfinite(bd_h).all()
+    hit = float((bi_h == planted).mean())
+    print("paper-shaped: %.1f %% of the planted orientations recovered" % (100 * hit))
+    assert hit >= 0.95                                         # the rest: another of 1.2 M orientations is closer still
+    rows = rng.choice(cfg.n_img, 32, replace=False)
+    subset = np.unique(np.concatenate([bi_h[rows], rng.integers(0, cfg.M, 2048)]))
+    S_sub = ctx.spf_slice(_dev(refs[subset]), d_pix, spf.SPF_OUT_INTENSITY, scale=alpha).cpu().numpy()
+    oi, od, osd, _ = orc.match(images[torch.from_numpy(rows).cuda()].cpu().numpy(), S_sub, mask)
+    assert np.all(np.abs(bd_h[rows] - od) <= DIST_TOL * od)
+    assert np.all((subset[oi] == bi_h[rows]) | ((osd - od) <= DIST_TOL * od))
