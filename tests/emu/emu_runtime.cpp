@@ -12,6 +12,9 @@
 
 dim3 threadIdx, blockIdx, blockDim, gridDim;
 
+#include <chrono>
+double emu_now_ms() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
+
 namespace emu {
 
 struct Fiber {
