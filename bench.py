@@ -241,6 +241,13 @@ def run_spf(args, cfg):
     # workload generation (outside every timed region): Poisson means come from the CUDA slicer at the
     # truth orientations -- inputs, not a correctness reference
     ctx.spf_prepare_model(d_model)
+    if not args.native and not args.reference_kernels_only:
+        # Among the CLASSIC-CUDA slicers (no TMA, mbarrier or tcgen05 in either) the C library checks the warp-per-point
+        # gather against the reference gather on this model and switches it on if it agrees and is faster (spf_selftest).
+        st = ctx.spf_selftest("slice_gcoop")
+        variants["slice_gcoop"] = st["passed"]
+        variants["slice_selftest"] = st["detail"]
+        variants["slice_impl"] = ctx.spf_get_option("slice_impl")
     slices = ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=1.0)
     alpha = photon_scale(slices, mask, cfg.photons)
     images = torch.empty((cfg.n_img, cfg.P), dtype=torch.float32, device=dev)
@@ -512,6 +519,8 @@ def main():
                     help="self-check the TMA / tcgen05 kernel variants in child processes and use the ones that pass "
                          "(opt-in until cleared on hardware; default: the library's default kernels only)")
     ap.add_argument("--no-autotune", action="store_true", help="(default behaviour now; kept for old command lines)")
+    ap.add_argument("--reference-kernels-only", action="store_true",
+                    help="skip even the in-process check of the classic-CUDA warp-per-point slicer: reference gather + CUDA-core matcher")
     args = ap.parse_args()
     if args.steps < 1:
         raise SystemExit("--steps must be >= 1")

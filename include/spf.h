@@ -227,12 +227,13 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  * Returns SPF_EINVAL for an unknown key or value.
  */
 SPF_API int spf_set_option(spf_ctx *ctx, const char *key, int64_t value);
+SPF_API int spf_get_option(const spf_ctx *ctx, const char *key, int64_t *value);   /* value [host]; SPF_EINVAL for an unknown key */
 
 /*
  * Device self-check of one kernel variant against this library's reference kernels, and the switch that turns a verified
  * variant on.  variant: "slice_gcoop" (slice_impl 3), "slice_coop" (slice_impl 2), "match_cg1", "match_cg2" (the tcgen05
  * matcher on single CTAs / CTA pairs).  Slicing variants slice the caller's own prepared model (read-only; SPF_ESTATE
- * before spf_prepare_model) at 16 seeded orientations x 4,096 pixels with the reference gather and with the variant
+ * before spf_prepare_model) at 64 seeded orientations x 16,384 pixels with the reference gather and with the variant
  * (bar: relative L2 <= 3e-6, all finite); matcher variants run two seeded cases, with and without a mask, against
  * spf_match_reference (bar: distances within 1e-4 d; without the refinement 1e-4 d + 2e-6 of the norms; argmin equal
  * outside near-ties).  A consistency check between two CUDA paths, not parity (tests/ hold every variant to the oracle).

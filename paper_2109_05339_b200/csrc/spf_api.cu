@@ -109,6 +109,17 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     return spf_set_err(ctx, SPF_EINVAL, "unknown option %s=%lld", key, (long long)value);
 }
 
+int spf_get_option(const spf_ctx *ctx, const char *key, int64_t *value) {
+    if (!ctx || !key || !value) return SPF_EINVAL;
+    const struct { const char *k; int v; } tab[] = {
+        {"slice_impl", ctx->opt_slice_impl}, {"force_complex_grid", ctx->opt_force_complex}, {"match_cta_group", ctx->opt_match_cta_group},
+        {"match_impl", ctx->opt_match_impl}, {"match_chunk_kblocks", ctx->opt_match_chunk_kb}, {"match_condition", ctx->opt_match_condition},
+        {"match_refine", ctx->opt_match_refine}, {"selftest_small", ctx->opt_selftest_small}, {"record_events", ctx->opt_record_events}};
+    for (const auto &e : tab)
+        if (!strcmp(key, e.k)) { *value = e.v; return SPF_OK; }
+    return SPF_EINVAL;
+}
+
 int spf_check_fault(spf_ctx *ctx, void *stream_) {
     if (!ctx) return SPF_EINVAL;
     SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));

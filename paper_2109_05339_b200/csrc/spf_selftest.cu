@@ -41,13 +41,14 @@ void say(spf_selftest_report *r, const char *fmt, ...) {
 float elapsed_ms(cudaEvent_t a, cudaEvent_t b) { float ms = 0.f; cudaEventSynchronize(b); cudaEventElapsedTime(&ms, a, b); return ms; }
 
 // ------------------------------------------------------------------------------------------ slicing variants
-// The caller's own prepared model is sliced (read-only) at 16 seeded orientations x a 64 x 64-pixel flat detector (3 x 24 x 24 with option "selftest_small") on
+// The caller's own prepared model is sliced (read-only) at 64 seeded orientations x a 128 x 128-pixel flat detector (1 M points, 8,192 blocks: long enough to time; 3 x 24 x 24
+// with option "selftest_small") on
 // the Ewald sphere (8 x 16 lattice patches with the layout promise, 0.9 Nyquist), once with the reference gather and
 // once with `impl`; complex output.  Bar: relative L2 difference <= 3e-6 (the two differ in how the kernel weights are
 // evaluated -- polynomial fit vs exp / sqrt -- and in summation order), every value finite.
 int selftest_slice(spf_ctx *ctx, int impl, spf_selftest_report *rep, cudaStream_t st) {
     if (!ctx->prepared) return spf_set_err(ctx, SPF_ESTATE, "spf_selftest(slice variant) slices the caller's model: call spf_prepare_model first");
-    const int edge = ctx->opt_selftest_small ? 24 : 64, P = edge * edge, M = ctx->opt_selftest_small ? 3 : 16;
+    const int edge = ctx->opt_selftest_small ? 24 : 128, P = edge * edge, M = ctx->opt_selftest_small ? 3 : 64;
     std::vector<float> pix((size_t)P * 3), quats((size_t)M * 4);
     double qmax = 0.0;
     for (int r = 0; r < edge; ++r)

@@ -103,6 +103,10 @@ def transform(name, text):
 
 
 def build_emu(force: bool = False) -> str:
+    global LIB
+    asan = os.environ.get("SPF_EMU_ASAN", "0") == "1"      # AddressSanitizer build (run python under LD_PRELOAD=libasan.so)
+    if asan:
+        LIB = os.path.join(HERE, "libspf_emu_asan.so")
     srcs = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(HERE, f) for f in EMU_FILES]
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(p) for p in srcs):
         return LIB
@@ -116,9 +120,11 @@ def build_emu(force: bool = False) -> str:
     # pipeline that deadlocks under emulation reports SPF_EFAULT within seconds
     flags = ["-O1", "-g", "-std=c++17", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing", "-DSPF_EMU", "-DSPF_DEBUG",
              "-DSPF_WAIT_CYCLES=(1ll<<22)", "-DSPF_DRAIN_CYCLES=(1ll<<8)", "-I" + HERE, "-I" + GEN, "-Wno-unused-value"]
+    if asan:
+        flags += ["-fsanitize=address", "-fno-omit-frame-pointer"]
     objs, procs = [], []
     for f in [os.path.join(GEN, s.replace(".cu", ".cpp")) for s in SOURCES] + [os.path.join(HERE, "emu_runtime.cpp")]:
-        o = os.path.join(GEN, os.path.basename(f) + ".o")
+        o = os.path.join(GEN, os.path.basename(f) + (".asan.o" if asan else ".o"))
         objs.append(o)
         procs.append((f, subprocess.Popen(["g++", *flags, "-c", f, "-o", o], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     bad = False
@@ -129,7 +135,7 @@ def build_emu(force: bool = False) -> str:
             print("---- g++ %s ----\n%s" % (f, out[-6000:]))
     if bad:
         raise RuntimeError("emulator build failed")
-    subprocess.run(["g++", "-shared", "-o", LIB + ".tmp", *objs], check=True)
+    subprocess.run(["g++", "-shared", *(["-fsanitize=address"] if asan else []), "-o", LIB + ".tmp", *objs], check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB
 

@@ -78,7 +78,7 @@ def dry_run(sm_count=4):
     import ctypes as C
     proxy = _TorchProxy(real_torch)
     saved = {"lib_path": b.LIB_PATH, "lib": b._lib, "dev": b._dev, "stream": b._stream, "btorch": b.torch,
-             "sys_torch": sys.modules["torch"], "t_cuda": real_torch.Tensor.cuda, "t_pin": real_torch.Tensor.pin_memory,
+             "selftest": b.SpfContext.spf_selftest, "sys_torch": sys.modules["torch"], "t_cuda": real_torch.Tensor.cuda, "t_pin": real_torch.Tensor.pin_memory,
              "t_to": real_torch.Tensor.to}
 
     def _dev(t, dtype, what):
@@ -94,7 +94,12 @@ def dry_run(sm_count=4):
             k["device"] = "cpu"
         return saved["t_to"](self, *a, **k)
 
+    def _selftest_small(self, variant):          # the emulator cannot afford the check's full-size cases
+        self.spf_set_option("selftest_small", 1)
+        return saved["selftest"](self, variant)
+
     try:
+        b.SpfContext.spf_selftest = _selftest_small
         b.LIB_PATH, b._lib = build_emu(), None
         b._dev, b._stream, b.torch = _dev, (lambda device: None), proxy
         lib = b.load_library()
@@ -106,6 +111,7 @@ def dry_run(sm_count=4):
         real_torch.Tensor.to = _to
         yield proxy
     finally:
+        b.SpfContext.spf_selftest = saved["selftest"]
         b.LIB_PATH, b._lib, b._dev, b._stream, b.torch = saved["lib_path"], saved["lib"], saved["dev"], saved["stream"], saved["btorch"]
         sys.modules["torch"] = saved["sys_torch"]
         real_torch.Tensor.cuda, real_torch.Tensor.pin_memory, real_torch.Tensor.to = saved["t_cuda"], saved["t_pin"], saved["t_to"]

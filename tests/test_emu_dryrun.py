@@ -25,7 +25,7 @@ def test_bench_cuda_arm_runs_end_to_end_on_tiny():
     host-buffer call, oracle baseline, one JSON line with every key the contract names."""
     import bench
     args = argparse.Namespace(gpus=1, steps=2, warmup=3, impl="spf", config="tiny", no_cpu_baseline=False, no_e2e=False,
-                              native=False, no_autotune=False)
+                              native=False, no_autotune=False, reference_kernels_only=False)
     out = io.StringIO()
     with dry_run(), redirect_stdout(out):
         bench.run_spf(args, bench.CONFIGS["tiny"])
@@ -38,6 +38,7 @@ def test_bench_cuda_arm_runs_end_to_end_on_tiny():
     assert j["n_gpus"] == 1 and j["steps"] == 2 and j["value"] > 0 and j["vs_baseline"] is None
     assert j["config"]["workload"] == "tiny" and j["config"]["w"] == 8
     assert j["config"]["kernel_variants"]["match"].startswith("cuda_core")
+    assert j["config"]["kernel_variants"]["selfcheck"]["slice_gcoop"] is True     # the classic warp-per-point slicer was checked in-process
     assert j["roofline"]["bound"] in ("smem", "alu") and j["roofline"]["frac"] > 0
     assert j["kernels"]["match_prep"]["roofline"] is None          # CUDA-core matcher: no operand preparation
     assert j["gpu_launches"] == 2 * 6                               # 6 kernels of the library per step on the defaults
