@@ -181,3 +181,33 @@ def test_tcgen05_variants_and_cuda_core_matcher_agree_on_counts(spf, verified):
     assert np.allclose(res["simt"][1], res["cg1"][1], rtol=1e-4)
     if "cg2" in res:
         assert np.allclose(res["cg1"][1], res["cg2"][1], rtol=2e-6)
+
+
+def test_tcgen05_accumulator_rounding_at_k_65536(spf, verified):
+    """Does sm_100a's tensor-core accumulator round to nearest or truncate?  (decides the default of
+    `match_chunk_kblocks`.)  Paper-scale statistics, K = 65,536 pixels, 128 images x 256 slices, the contraction's own
+    a_i + b_m - 2 G (match_refine = 0): once with all of K accumulated in TMEM (chunk 0), once with the library's chunks
+    of 32 K blocks.  The CPU replay predicts 1.9e-4 (truncating) or <= 5e-6 (nearest) for chunk 0 and <= 1e-5 for chunks
+    of 32 under either rounding.  Only the library's setting is held to the bar; the other number is the measurement."""
+    _require(verified, "match_cg1")
+    from spf_inputs import make_mask, poisson_images, surrogate_slices
+    cfg = CONFIGS["paper_scale"]
+    pix = make_detector(cfg.panels, cfg.panel_edge)
+    mask = make_mask(cfg.panels, cfg.panel_edge, cfg.masked_frac)
+    S = surrogate_slices(256, pix)
+    S *= np.float32(cfg.photons / float(S.sum(axis=1).mean()))
+    I = poisson_images(S[np.arange(128) * 2 % 256])
+    oi, od, _, _ = orc.match(I, S, mask)
+    ctx = spf.SpfContext(8)
+    base.set_match_variant(ctx, "cg2" if verified["match_cg2"]["ok"] else "cg1")
+    ctx.spf_set_option("match_refine", 0)
+    worst = {}
+    for chunk in (0, 32):
+        ctx.spf_set_option("match_chunk_kblocks", chunk)
+        bi, bd = ctx.spf_match(_dev(I), _dev(S), _dev(mask))
+        ctx.spf_check_fault()
+        assert np.array_equal(bi.cpu().numpy(), oi)
+        worst[chunk] = float(np.max(np.abs(bd.cpu().numpy() - od) / od))
+    print("K = 65,536 accumulation, worst relative distance error: whole K in TMEM %.2e, chunks of 32 K blocks %.2e"
+          % (worst[0], worst[32]))
+    assert worst[32] <= 2e-5
