@@ -49,6 +49,23 @@ def _peaks():
                 "source": "fallback"}
 
 
+def measure_device_peaks(ctx):
+    """The SM-side denominators, measured on this device in this run (spf_microbench, csrc/spf_microbench.cu; SURVEY.md
+    section 8(d)): aggregate shared-memory load bandwidth (the slicing roofline's peak) and L2 -> SM bandwidth, plus an HBM copy
+    as a sanity check against MEASURED_PEAKS.json.  A failure leaves the nominal figures in place and says so."""
+    out = {}
+    try:
+        lds = {k: ctx.spf_microbench(k) for k in ("lds32", "lds128")}
+        out["lds_gbs"] = max(lds.values())
+        out["lds_gbs_by_load_width"] = lds
+        out["l2_to_sm_gbs"] = ctx.spf_microbench("l2")
+        out["hbm_copy_gbs_this_run"] = ctx.spf_microbench("hbm_copy")
+        out["sm_side_source"] = "measured in this run by spf_microbench (best of 3 after a warm-up, CUDA events)"
+    except Exception as e:      # the rooflines then fall back to the nominal SM-side figures
+        out["sm_side_source"] = "nominal (spf_microbench failed: %s)" % repr(e)[:120]
+    return out
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled every 200 ms during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -234,6 +251,7 @@ def run_spf(args, cfg):
                 {"slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False,
                  "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
     info = ctx.info
+    measured = measure_device_peaks(ctx) if rank == 0 or world > 1 else {}
     d_model = torch.from_numpy(model).to(dev)
     d_pix, d_refs = torch.from_numpy(pix).to(dev), torch.from_numpy(refs).to(dev)
     d_mask = None if mask is None else torch.from_numpy(mask).to(dev)
@@ -328,6 +346,7 @@ def run_spf(args, cfg):
     hit = float((best_idx.cpu().numpy()[sel] == planted[sel]).mean()) if sel.any() else None
 
     peaks = _peaks()
+    peaks.update(measured)
     kern = roofline_objects(cfg, info, k_ms, products, peaks, clk)
     dominant = max(("slice", "gemm"), key=lambda n: kern[n]["ms"])
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -397,14 +416,17 @@ def roofline_objects(cfg, info, k_ms, products, peaks, clk):
     # SM-side memory roofline (north_star's "memory roofline" as SURVEY.md section 8(d) reads it): every point needs
     # w^3 grid values (4 B real, 8 B complex) delivered from shared memory / L1 to a lane, against 128 B/clk/SM
     smem_bytes = pts * (w ** 3) * (4.0 if real else 8.0)
-    smem_peak = info.sm_count * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9                # GB/s
+    smem_nominal = info.sm_count * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9             # GB/s, the guide's 128 B/clk/SM at max clock
+    smem_peak = float(peaks.get("lds_gbs") or smem_nominal)                            # measured in this run when available
     smem_ach = smem_bytes / t_s / 1e9
     out["slice"] = {"ms": t_s * 1e3, "points_per_s": pts / t_s,
                     "roofline": {"kernel": "k_slice", "bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "GB/s",
                                  "frac": smem_ach / smem_peak, "traffic": None,
-                                 "peak_source": "SM-side memory: 148 SM x 128 B/clk x sm_max_mhz; algorithmic bytes = w^3 grid "
-                                                "values per point (DESIGN.md section 6.1); HBM and FMA-pipe figures beside it",
-                                 "frac_at_observed_clock": (smem_ach / (smem_peak * clk["sm_mhz"] / peaks["sm_max_mhz"])) if clk.get("sm_mhz") else None},
+                                 "peak_source": ("aggregate shared-memory load bandwidth measured in this run (spf_microbench)" if peaks.get("lds_gbs")
+                                                 else "NOMINAL 148 SM x 128 B/clk x sm_max_mhz (no measurement)") +
+                                                "; algorithmic bytes = w^3 grid values per point (DESIGN.md section 6.1); HBM and FMA-pipe figures beside it",
+                                 "peak_nominal": smem_nominal, "frac_of_nominal": smem_ach / smem_nominal,
+                                 "frac_of_nominal_at_observed_clock": (smem_ach / (smem_nominal * clk["sm_mhz"] / peaks["sm_max_mhz"])) if clk.get("sm_mhz") else None},
                     "alu": {"achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
                             "peak_source": "148 SM x 128 FMA lanes x 2 x sm_max_mhz"},
                     "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / t_s / 1e9, "peak_gbs": peaks["hbm_gbs"],

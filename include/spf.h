@@ -254,6 +254,15 @@ typedef struct {
 SPF_API int spf_selftest(spf_ctx *ctx, const char *variant, spf_selftest_report *report, void *stream);
 
 /*
+ * Measures one of the device figures the rooflines divide by (the SM-side peaks must be
+ * microbenchmarked, not taken from a data sheet).  what: "lds32" / "lds128" -- aggregate shared-memory load bandwidth with
+ * conflict-free 4-byte / 16-byte loads (all SMs, 4 blocks of 512 threads each); "l2" -- L2 -> SM read bandwidth (a 48 MB
+ * buffer streamed 20 times with L1-bypassing loads); "hbm_read" / "hbm_copy" -- 1 GB read twice / copied once.  Best of
+ * three timed repetitions after a warm-up, CUDA events on `stream`.  gb_per_s [host].  Synchronises.
+ */
+SPF_API int spf_microbench(spf_ctx *ctx, const char *what, double *gb_per_s, void *stream);
+
+/*
  * Watchdog.  Every wait on a hardware barrier inside the slicing and matching kernels is bounded
  * (about two seconds of SM clocks): a pipeline that stalls makes its block record a fault, raise the
  * context's device-global abort flag (every other block gives up at its next poll, blocks that start

@@ -21,7 +21,7 @@ EXPORTS = ["spf_version", "spf_status_string", "spf_plan_kernel_width", "spf_pla
            "spf_get_info", "spf_last_error", "spf_set_detector_layout", "spf_prepare_model", "spf_slice", "spf_match",
            "spf_match_workspace_bytes", "spf_match_reference", "spf_orientation_match_host", "spf_debug_deapodisation",
            "spf_debug_fine_grid", "spf_set_option", "spf_launch_count", "spf_last_kernel_ms", "spf_last_match_products",
-           "spf_check_fault", "spf_selftest", "spf_slice_match", "spf_slice_match_workspace_bytes", "spf_get_option"]
+           "spf_check_fault", "spf_selftest", "spf_slice_match", "spf_slice_match_workspace_bytes", "spf_get_option", "spf_microbench"]
 
 
 class SpfParams(C.Structure):
@@ -82,6 +82,7 @@ def load_library():
     lib.spf_debug_fine_grid.argtypes = [vp, vp, vp]
     lib.spf_set_option.argtypes = [vp, C.c_char_p, i64]
     lib.spf_get_option.argtypes = [vp, C.c_char_p, C.POINTER(i64)]
+    lib.spf_microbench.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double), vp]
     lib.spf_launch_count.argtypes = [vp]
     lib.spf_launch_count.restype = i64
     lib.spf_last_kernel_ms.argtypes = [vp, i32, C.POINTER(C.c_float)]
@@ -161,6 +162,12 @@ class SpfContext:
         v = C.c_int64()
         self._check(self._lib.spf_get_option(self._h, key.encode(), C.byref(v)))
         return int(v.value)
+
+    def spf_microbench(self, what: str) -> float:
+        """GB/s of one device figure (spf.h): "lds32", "lds128", "l2", "hbm_read", "hbm_copy"."""
+        v = C.c_double()
+        self._check(self._lib.spf_microbench(self._h, what.encode(), C.byref(v), _stream(self.device)))
+        return float(v.value)
 
     def spf_check_fault(self):
         """Synchronise the current stream; raise SpfError(SPF_EFAULT) if a kernel's watchdog gave up."""

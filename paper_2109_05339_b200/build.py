@@ -6,7 +6,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libspf.so")
-SOURCES = ["spf_api.cu", "spf_prepare.cu", "spf_slice.cu", "spf_match.cu", "spf_selftest.cu"]
+SOURCES = ["spf_api.cu", "spf_prepare.cu", "spf_slice.cu", "spf_match.cu", "spf_selftest.cu", "spf_microbench.cu"]
 HEADERS = ["spf_internal.cuh", "ptx_sm100.cuh", "spf_slice_math.cuh", "spf_match_math.cuh", os.path.join("..", "..", "include", "spf.h")]
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -18,7 +18,7 @@ ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2109_05339_b200", "csrc")
 GEN = os.path.join(HERE, "gen")
 LIB = os.path.join(HERE, "libspf_emu.so")
-SOURCES = ["spf_api.cu", "spf_prepare.cu", "spf_slice.cu", "spf_match.cu", "spf_selftest.cu"]
+SOURCES = ["spf_api.cu", "spf_prepare.cu", "spf_slice.cu", "spf_match.cu", "spf_selftest.cu", "spf_microbench.cu"]
 HEADERS = ["spf_internal.cuh", "ptx_sm100.cuh", "spf_slice_math.cuh", "spf_match_math.cuh"]
 EMU_FILES = ["cuda_emu.h", "ptx_emu.cuh", "emu_runtime.cpp", "build_emu.py"]
 

@@ -121,6 +121,7 @@ inline void __threadfence_system() {}
 inline void __threadfence_block() {}
 inline long long clock64() { return ++emu::g_ticks; }
 template <class T> inline T __ldg(const T *p) { return *p; }
+template <class T> inline T __ldcg(const T *p) { return *p; }
 inline uint32_t __float_as_uint(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
 inline float __uint_as_float(uint32_t u) { float f; memcpy(&f, &u, 4); return f; }
 inline size_t __cvta_generic_to_shared(const void *p) { return emu::shared_addr(p); }

@@ -78,7 +78,7 @@ def dry_run(sm_count=4):
     import ctypes as C
     proxy = _TorchProxy(real_torch)
     saved = {"lib_path": b.LIB_PATH, "lib": b._lib, "dev": b._dev, "stream": b._stream, "btorch": b.torch,
-             "selftest": b.SpfContext.spf_selftest, "sys_torch": sys.modules["torch"], "t_cuda": real_torch.Tensor.cuda, "t_pin": real_torch.Tensor.pin_memory,
+             "selftest": b.SpfContext.spf_selftest, "microbench": b.SpfContext.spf_microbench, "sys_torch": sys.modules["torch"], "t_cuda": real_torch.Tensor.cuda, "t_pin": real_torch.Tensor.pin_memory,
              "t_to": real_torch.Tensor.to}
 
     def _dev(t, dtype, what):
@@ -98,8 +98,12 @@ def dry_run(sm_count=4):
         self.spf_set_option("selftest_small", 1)
         return saved["selftest"](self, variant)
 
+    def _microbench_small(self, what):           # functional run only: the figure means nothing under emulation
+        self.spf_set_option("selftest_small", 1)
+        return saved["microbench"](self, what)
+
     try:
-        b.SpfContext.spf_selftest = _selftest_small
+        b.SpfContext.spf_selftest, b.SpfContext.spf_microbench = _selftest_small, _microbench_small
         b.LIB_PATH, b._lib = build_emu(), None
         b._dev, b._stream, b.torch = _dev, (lambda device: None), proxy
         lib = b.load_library()
@@ -111,7 +115,7 @@ def dry_run(sm_count=4):
         real_torch.Tensor.to = _to
         yield proxy
     finally:
-        b.SpfContext.spf_selftest = saved["selftest"]
+        b.SpfContext.spf_selftest, b.SpfContext.spf_microbench = saved["selftest"], saved["microbench"]
         b.LIB_PATH, b._lib, b._dev, b._stream, b.torch = saved["lib_path"], saved["lib"], saved["dev"], saved["stream"], saved["btorch"]
         sys.modules["torch"] = saved["sys_torch"]
         real_torch.Tensor.cuda, real_torch.Tensor.pin_memory, real_torch.Tensor.to = saved["t_cuda"], saved["t_pin"], saved["t_to"]

@@ -82,6 +82,9 @@ def test_roofline_arithmetic_matches_design_md():
     k = bench.roofline_objects(cfg, info, k_ms, 2, peaks, {"sm_mhz": 1312.0})
     s = k["slice"]["roofline"]
     assert s["bound"] == "smem" and s["unit"] == "GB/s" and abs(s["peak"] - 148 * 128 * 1.965e9 / 1e9) < 1e-6
+    assert "NOMINAL" in s["peak_source"] and abs(s["frac_of_nominal"] - s["frac"]) < 1e-12
+    km = bench.roofline_objects(cfg, info, k_ms, 2, dict(peaks, lds_gbs=30000.0), {"sm_mhz": 1312.0})["slice"]["roofline"]
+    assert km["peak"] == 30000.0 and "measured in this run" in km["peak_source"] and abs(km["frac"] - s["achieved"] / 30000.0) < 1e-12
     assert abs(s["achieved"] - 10_000 * 65_536 * 343 * 4 / 12e-3 / 1e9) < 1e-3
     assert abs(s["frac"] - s["achieved"] / s["peak"]) < 1e-12
     alu = k["slice"]["alu"]

@@ -45,6 +45,8 @@ def test_bench_cuda_arm_runs_end_to_end_on_tiny():
     assert j["e2e"]["value"] > 0 and j["e2e"]["h2d_bytes_per_step"] > 16 * 1024 * 4 and j["e2e"]["d2h_bytes_per_step"] == 16 * 8
     assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["value"] > 0
     assert j["planted_hit_rate"] is not None
+    assert j["peaks"]["lds_gbs"] > 0 and j["peaks"]["l2_to_sm_gbs"] > 0 and "measured in this run" in j["peaks"]["sm_side_source"]
+    assert "measured in this run" in j["kernels"]["slice"]["roofline"]["peak_source"]
 
 
 def test_smoke_runs_on_the_emulator():
