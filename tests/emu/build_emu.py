@@ -20,7 +20,8 @@ GEN = os.path.join(HERE, "gen")
 LIB = os.path.join(HERE, "libspf_emu.so")
 SOURCES = ["spf_api.cu", "spf_prepare.cu", "spf_slice.cu", "spf_match.cu", "spf_selftest.cu", "spf_microbench.cu"]
 HEADERS = ["spf_internal.cuh", "ptx_sm100.cuh", "spf_slice_math.cuh", "spf_match_math.cuh"]
-EMU_FILES = ["cuda_emu.h", "ptx_emu.cuh", "emu_runtime.cpp", "build_emu.py"]
+EMU_FILES = ["cuda_emu.h", "ptx_emu.cuh", "emu_runtime.cpp", "build_emu.py", os.path.join("selftest", "emu_faults.cu")]
+EXTRA = [os.path.join(HERE, "selftest", "emu_faults.cu")]     # deliberately broken kernels: the emulator's own self-test
 
 
 def _match_close(text, start, open_ch, close_ch):
@@ -116,6 +117,11 @@ def build_emu(force: bool = False) -> str:
             text = transform(f, fh.read())
         with open(os.path.join(GEN, f.replace(".cu", ".cpp") if f.endswith(".cu") else f), "w") as fh:
             fh.write(text)
+    for f in EXTRA:
+        with open(f) as fh:
+            text = transform(os.path.basename(f), fh.read())
+        with open(os.path.join(GEN, os.path.basename(f).replace(".cu", ".cpp")), "w") as fh:
+            fh.write(text)
     # the watchdog's bounds count emulator ticks (one per fiber switch), not SM clocks: keep them small so that a
     # pipeline that deadlocks under emulation reports SPF_EFAULT within seconds
     flags = ["-O1", "-g", "-std=c++17", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing", "-DSPF_EMU", "-DSPF_DEBUG",
@@ -123,7 +129,7 @@ def build_emu(force: bool = False) -> str:
     if asan:
         flags += ["-fsanitize=address", "-fno-omit-frame-pointer"]
     objs, procs = [], []
-    for f in [os.path.join(GEN, s.replace(".cu", ".cpp")) for s in SOURCES] + [os.path.join(HERE, "emu_runtime.cpp")]:
+    for f in [os.path.join(GEN, s.replace(".cu", ".cpp")) for s in SOURCES] + [os.path.join(GEN, os.path.basename(e).replace(".cu", ".cpp")) for e in EXTRA] + [os.path.join(HERE, "emu_runtime.cpp")]:
         o = os.path.join(GEN, os.path.basename(f) + (".asan.o" if asan else ".o"))
         objs.append(o)
         procs.append((f, subprocess.Popen(["g++", *flags, "-c", f, "-o", o], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))

@@ -30,6 +30,7 @@ Cta *cur_cta = nullptr;
 int g_cluster_size = 1;
 long long g_ticks = 0;
 int g_sm_count = 4;
+long g_counters[4] = {0, 0, 0, 0};   // [0] bulk tensor copies, [1] tcgen05.mma, [2] kernel launches, [3] fiber switches
 
 namespace {
 constexpr size_t STACK_BYTES = 256 * 1024;
@@ -41,7 +42,8 @@ std::vector<size_t> dyn_cap;
 const std::function<void()> *body_fn = nullptr;
 int cluster_alive = 0, cluster_arrived = 0;
 unsigned cluster_gen = 0;
-std::deque<std::function<void()>> async_q;
+struct AsyncOp { long ready; std::function<void()> fn; };
+std::deque<AsyncOp> async_q;        // FIFO: an operation lands no earlier than `ready` (in fiber switches) and never before its predecessors
 std::string g_fault;
 uint32_t rng_state = 12345u;
 std::vector<const void *> static_shared;   // static __shared__ objects whose address was taken (mbarriers of k_slice)
@@ -67,10 +69,10 @@ void fiber_entry() {
 }
 
 void drain_async(bool all) {
-    // a few deferred operations per scheduler step (never none for long: progress is guaranteed)
-    int n = all ? (int)async_q.size() : (int)(rnd() % 3u);
-    while (n-- > 0 && !async_q.empty()) {
-        std::function<void()> op = std::move(async_q.front());
+    // deferred operations land in issue order, each no earlier than its own latency after it was issued (a few hundred to
+    // a few thousand fiber switches): a consumer that does not wait for the barrier reads poison, not data
+    while (!async_q.empty() && (all || async_q.front().ready <= g_counters[3])) {
+        std::function<void()> op = std::move(async_q.front().fn);
         async_q.pop_front();
         op();
     }
@@ -131,8 +133,7 @@ const uint64_t *warp_collective(uint64_t v) {
     return w.vals[g & 1];
 }
 
-long g_counters[4] = {0, 0, 0, 0};   // [0] bulk tensor copies, [1] tcgen05.mma, [2] kernel launches, [3] fiber switches
-void async_push(std::function<void()> op) { async_q.push_back(std::move(op)); }
+void async_push(std::function<void()> op) { async_q.push_back(AsyncOp{g_counters[3] + 300 + (long)(rnd() % 3000u), std::move(op)}); }
 
 uint32_t shared_addr(const void *p) {
     const uint8_t *b = (const uint8_t *)p;
