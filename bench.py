@@ -248,7 +248,7 @@ def run_spf(args, cfg):
     # device self-check passes in a child process (paper_2109_05339_b200/selfcheck.py).  Opt-in until those kernels
     # have been cleared on hardware: the default run never launches an unverified kernel.
     variants = (ctx.spf_autotune() if args.native else
-                {"slice_coop": False, "slice_gcoop": False, "match_cg1": False, "match_cg2": False,
+                {"slice_coop": False, "slice_gcoop": False, "slice_coop_ld": False, "match_cg1": False, "match_cg2": False,
                  "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
     info = ctx.info
     measured = measure_device_peaks(ctx) if rank == 0 or world > 1 else {}
@@ -262,9 +262,12 @@ def run_spf(args, cfg):
     if not args.native and not args.reference_kernels_only:
         # Among the CLASSIC-CUDA slicers (no TMA, mbarrier or tcgen05 in either) the C library checks the warp-per-point
         # gather against the reference gather on this model and switches it on if it agrees and is faster (spf_selftest).
-        st = ctx.spf_selftest("slice_gcoop")
-        variants["slice_gcoop"] = st["passed"]
-        variants["slice_selftest"] = st["detail"]
+        # (3: straight from global memory; 4: from a tile staged by cp.async).  The fastest one that agrees is used.
+        variants["slice_selftest"] = {}
+        for v in ("slice_gcoop", "slice_coop_ld"):
+            st = ctx.spf_selftest(v)
+            variants[v] = st["passed"]
+            variants["slice_selftest"][v] = st["detail"]
         variants["slice_impl"] = ctx.spf_get_option("slice_impl")
     slices = ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=1.0)
     alpha = photon_scale(slices, mask, cfg.photons)
@@ -357,7 +360,8 @@ def run_spf(args, cfg):
                        "n_img_per_gpu": cfg.n_img, "eps": cfg.eps, "masked_frac": cfg.masked_frac,
                        "grid_is_real": bool(info.grid_is_real),
                        "kernel_variants": {"slice": {1: "global_gather, thread per point",
-                                                     2: "tma_staged, warp per point", 3: "global_gather, warp per point"}[variants["slice_impl"]],
+                                                     2: "tma_staged, warp per point", 3: "global_gather, warp per point",
+                                                     4: "cp_async_staged, warp per point"}[variants["slice_impl"]],
                                            "match": ("tcgen05 cta_group::%d" % variants["match_cta_group"]) if variants["match_impl"] == 0
                                                     else "cuda_core difference form (library default; tcgen05 variant %s)" % ("failed its self-check" if args.native else "not requested"),
                                            "selfcheck": variants},

@@ -206,7 +206,9 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *                      with no bank conflicts and a shuffle butterfly adds the partial sums (w <= 8; blocks whose box
  *                      does not fit the tile, and every block at w = 10, run as 3);
  *                  3 = the warp-per-point gather straight from global memory (no TMA, mbarrier or tile;
- *                      8 x 8 window at w = 8, 16-cell window at w = 10)
+ *                      8 x 8 window at w = 8, 16-cell window at w = 10);
+ *                  4 = as 2, the tile staged by cp.async (16-byte pieces copied by every thread, block barrier) instead of
+ *                      TMA: classic CUDA only, the staged gather for a device on which the TMA path is not cleared
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
  *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused norm-add + argmin epilogue (the product);
  *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused
@@ -231,7 +233,7 @@ SPF_API int spf_get_option(const spf_ctx *ctx, const char *key, int64_t *value);
 
 /*
  * Device self-check of one kernel variant against this library's reference kernels, and the switch that turns a verified
- * variant on.  variant: "slice_gcoop" (slice_impl 3), "slice_coop" (slice_impl 2), "match_cg1", "match_cg2" (the tcgen05
+ * variant on.  variant: "slice_gcoop" (slice_impl 3), "slice_coop_ld" (slice_impl 4), "slice_coop" (slice_impl 2), "match_cg1", "match_cg2" (the tcgen05
  * matcher on single CTAs / CTA pairs).  Slicing variants slice the caller's own prepared model (read-only; SPF_ESTATE
  * before spf_prepare_model) at 64 seeded orientations x 16,384 pixels with the reference gather and with the variant
  * (bar: relative L2 <= 3e-6, all finite); matcher variants run two seeded cases, with and without a mask, against

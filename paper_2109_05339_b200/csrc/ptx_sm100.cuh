@@ -79,6 +79,14 @@ __device__ __forceinline__ void abort_drain() {
     while (clock64() - t0 < SPF_DRAIN_CYCLES) { }
 }
 
+// ---------------------------------------------------------------- cp.async (Ampere-style, no mbarrier, no tensor map)
+// 16 bytes global -> shared without a register round trip (SASS LDGSTS), L1 bypassed; dst and src 16-byte aligned
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+// all cp.async of this thread issued so far have landed when this returns (other threads: follow with a block barrier)
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // ---------------------------------------------------------------- TMA
 __device__ __forceinline__ void prefetch_tensormap(const void *map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");

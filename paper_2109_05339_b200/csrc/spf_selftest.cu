@@ -221,8 +221,8 @@ extern "C" int spf_selftest(spf_ctx *ctx, const char *variant, spf_selftest_repo
     cudaStream_t st = (cudaStream_t)stream_;
     SPF_CUDA(ctx, cudaSetDevice(ctx->prm.device));
     int rc;
-    if (!strcmp(variant, "slice_gcoop") || !strcmp(variant, "slice_coop")) {
-        const int impl = !strcmp(variant, "slice_coop") ? 2 : 3;
+    if (!strcmp(variant, "slice_gcoop") || !strcmp(variant, "slice_coop") || !strcmp(variant, "slice_coop_ld")) {
+        const int impl = !strcmp(variant, "slice_coop") ? 2 : (!strcmp(variant, "slice_coop_ld") ? 4 : 3);
         if ((rc = selftest_slice(ctx, impl, report, st))) return rc;
         if (report->passed) {
             // among the verified slicers the one this check timed fastest is switched on (never a slower one)
@@ -240,5 +240,5 @@ extern "C" int spf_selftest(spf_ctx *ctx, const char *variant, spf_selftest_repo
         }
         return SPF_OK;
     }
-    return spf_set_err(ctx, SPF_EINVAL, "spf_selftest: unknown variant %s (slice_gcoop, slice_coop, match_cg1, match_cg2)", variant);
+    return spf_set_err(ctx, SPF_EINVAL, "spf_selftest: unknown variant %s (slice_gcoop, slice_coop_ld, slice_coop, match_cg1, match_cg2)", variant);
 }

@@ -39,6 +39,7 @@ struct SliceArgs {
     double inv_nf;
     float beta;
     uint32_t cap_bytes;     // dynamic shared memory available for the tile
+    int stage_mode;         // IMPL_COOP: 0 = tile staged by TMA (bulk tensor copies + mbarrier), 1 = by cp.async (classic CUDA)
     uint32_t *fault;        // context fault record (host-mapped): written when the tile wait gives up
     uint32_t *abort_flag;   // context abort flag (device memory): set by the first wait that gives up, read by every block
     float coef[SPF_MAX_W][SPF_MAX_DEG + 1];  // phi at tap t as a polynomial in u = 2 (f + w/2) - 1
@@ -66,7 +67,10 @@ __device__ __forceinline__ void store_out(const SliceArgs &a, int64_t m, int64_t
 // of a warp are scattered over the tile and every load replays ~3.8 times on bank conflicts -- 41 wavefronts per
 // point against 18 here, tests/test_hostsim_slice_math.py::test_bank_conflicts... -- so it could not reach half of
 // the shared-memory roofline by construction and was deleted.)
-enum { IMPL_GLOBAL = 1, IMPL_COOP = 2, IMPL_GCOOP = 3 };
+//   IMPL_COOP_LD 4  IMPL_COOP's kernel with the tile staged by cp.async (16-byte pieces, every thread copies) instead of
+//                   TMA: Ampere-style classic CUDA, no tensor map, no mbarrier -- the staged gather for a device on which
+//                   the TMA path has not been cleared.  The box starts at a multiple of 4 cells along z (16-byte pieces).
+enum { IMPL_GLOBAL = 1, IMPL_COOP = 2, IMPL_GCOOP = 3, IMPL_COOP_LD = 4 };
 #define SPF_COOP_WTS_BYTES (SPF_PATCH * SPF_COOP_STRIDE * 4)   // 14,336 = 112 x 128
 
 // The cooperative gather of one warp over its 32 points (variants 2 and 3).  `tile` is the staged box in
@@ -178,6 +182,9 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         }
         __syncthreads();
         lox = s_lo[0]; loy = s_lo[1]; loz = s_lo[2];
+        // cp.async staging copies 16-byte pieces: the box starts at a multiple of 4 cells along z (rows of the padded grid
+        // are 16-byte aligned: sz is a multiple of 4), at most 3 cells wider than the tight box
+        if (a.stage_mode == 1) loz &= ~3;
         // a patch with no pixel at all (cannot happen with the tables build_patches makes) has lo > hi: not staged
         const bool any = s_hi[0] >= lox;
         const int Lx = any ? s_hi[0] - lox + w : 0, Ly = any ? s_hi[1] - loy + w : 0, Lz = any ? s_hi[2] - loz + w : 0;
@@ -195,7 +202,22 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
             assert(lox >= 0 && loy >= 0 && loz >= 0 && lox + Lx <= a.np && loy + Ly <= a.np && loz + Lz <= a.sz);
         }
 #endif
-        if (staged && tid < 32) {
+        if (staged && a.stage_mode == 1) {
+            // classic staging: every thread copies 16-byte pieces of the box, row by row (a warp covers 512 consecutive
+            // bytes of a row or of neighbouring rows); pieces beyond the grid (rows >= np, cells >= sz) are zero-filled,
+            // which is what the TMA path's out-of-bounds fill gives
+            const int q_per_row = bz * E / 4, pieces = Lx * g.by * q_per_row;
+            const uint32_t dst0 = ptx::smem_u32(s_tile);
+            for (int idx = tid; idx < pieces; idx += SPF_PATCH) {
+                const int q = idx % q_per_row, y = (idx / q_per_row) % g.by, x = idx / (q_per_row * g.by);
+                const uint32_t dst = dst0 + (uint32_t)(((x * S1 + y * bz) * E + 4 * q) * 4);
+                const int gy = loy + y, gz4 = loz * E + 4 * q;
+                if (gy < a.np && gz4 + 3 < a.sz * E)
+                    ptx::cp_async_16(dst, a.grid + ((size_t)((size_t)(lox + x) * a.np + gy) * a.sz) * E + gz4);
+                else
+                    *reinterpret_cast<float4 *>(s_tile + (dst - dst0)) = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        } else if (staged && tid < 32) {
             const uint32_t bar = ptx::smem_u32(&s_bar);
             if (tid == 0) ptx::mbar_expect_tx(bar, (uint32_t)(Lx * g.by * bz * CELL));
             __syncwarp();
@@ -236,8 +258,12 @@ __global__ void __launch_bounds__(SPF_PATCH, (IMPL == IMPL_GLOBAL || IMPL == IMP
         }
         __syncwarp();
     }
+    if (STAGED && staged && a.stage_mode == 1) {
+        ptx::cp_async_wait_all();
+        __syncthreads();          // every thread's pieces have landed
+    }
     if (STAGED && staged) {
-        if (!ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort, a.abort_flag)) {
+        if (a.stage_mode == 0 && !ptx::mbar_wait(ptx::smem_u32(&s_bar), 0, &s_abort, a.abort_flag)) {
             if (tid == 0) {
                 a.fault[1] = blockIdx.x; a.fault[2] = (uint32_t)patch; a.fault[3] = (uint32_t)(W * 10 + (REAL ? 1 : 0) + 100 * IMPL);
                 a.fault[0] = SPF_FAULT_SLICE;
@@ -320,11 +346,11 @@ template <bool REAL, int OUTK>
 int launch_slice_w(spf_ctx *ctx, SliceArgs &args, int impl, cudaStream_t st) {
     switch (ctx->w) {
         case 8:    // eps = 1e-6: the 8 x 8 window is exactly the kernel's footprint
-            if (impl == IMPL_COOP) return launch_slice<8, REAL, OUTK, IMPL_COOP>(ctx, args, st);
+            if (impl == IMPL_COOP || impl == IMPL_COOP_LD) return launch_slice<8, REAL, OUTK, IMPL_COOP>(ctx, args, st);
             if (impl == IMPL_GCOOP) return launch_slice<8, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
             return launch_slice<8, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         case 10:   // 10 x 10 window: the staged 8 x 8 form does not apply, variants 2 and 3 both walk global memory (16-cell window)
-            if (impl == IMPL_COOP || impl == IMPL_GCOOP) return launch_slice<10, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
+            if (impl == IMPL_COOP || impl == IMPL_COOP_LD || impl == IMPL_GCOOP) return launch_slice<10, REAL, OUTK, IMPL_GCOOP>(ctx, args, st);
             return launch_slice<10, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);
         default: return launch_slice<0, REAL, OUTK, IMPL_GLOBAL>(ctx, args, st);  // any other width: runtime-w global gather
     }
@@ -359,6 +385,7 @@ extern "C" int spf_slice(spf_ctx *ctx, const float *quats, int64_t M, const floa
     args.deg = spfm::fit_kernel_polys(ctx->w, ctx->beta, args.coef);
     args.maps = real ? ctx->maps_r : ctx->maps_c;
     args.fault = ctx->d_fault; args.abort_flag = ctx->d_abort;
+    args.stage_mode = ctx->opt_slice_impl == IMPL_COOP_LD ? 1 : 0;
     const int impl = ctx->opt_slice_impl;
     if (impl == IMPL_COOP && ctx->w <= 8 && !ctx->maps_ok)
         return spf_set_err(ctx, SPF_ECUDA, "spf_slice: slice_impl %d needs the TMA tensor maps, which could not be encoded: %s", impl,

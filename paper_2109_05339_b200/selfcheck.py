@@ -34,8 +34,8 @@ import sys
 import time
 
 # least machinery first: classic CUDA (no TMA / mbarrier / tcgen05), then TMA + mbarrier, then tcgen05, CTA pairs last
-VARIANTS = ("slice_gcoop", "slice_coop", "match_cg1", "match_cg2")
-SLICE_IMPL = {"slice_coop": 2, "slice_gcoop": 3}
+VARIANTS = ("slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2")
+SLICE_IMPL = {"slice_coop": 2, "slice_gcoop": 3, "slice_coop_ld": 4}
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
 

@@ -133,6 +133,7 @@ const uint64_t *warp_collective(uint64_t v) {
     return w.vals[g & 1];
 }
 
+void drain_all_async() { drain_async(true); }
 void async_push(std::function<void()> op) { async_q.push_back(AsyncOp{g_counters[3] + 300 + (long)(rnd() % 3000u), std::move(op)}); }
 
 uint32_t shared_addr(const void *p) {

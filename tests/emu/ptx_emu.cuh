@@ -29,6 +29,7 @@ std::unordered_map<uint32_t, MBar> &mbar_table();   // keyed by shared address; 
 MBar *mbar_at(uint32_t addr, const char *what);
 void mbar_check(MBar *m);
 void tma_copy(uint32_t dst, const CUtensorMap *map, int nd, const int *crd, uint32_t bar);
+void drain_all_async();
 void umma(int cg, uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate);
 }  // namespace emu
 
@@ -60,6 +61,13 @@ inline bool mbar_try_wait(uint32_t bar, uint32_t parity) {
     if (!ready) emu::yield();
     return ready;
 }
+
+// cp.async: deferred like every other asynchronous copy; wait_all drains the queue (all threads' copies: a superset)
+inline void cp_async_16(uint32_t dst, const void *src) {
+    if ((dst & 15u) || ((uintptr_t)src & 15u)) emu::fault("cp.async 16: unaligned address (shared 0x%x, global %p)", dst, src);
+    emu::async_push([=]() { void *d = emu::shared_ptr(dst); if (d) memcpy(d, src, 16); });
+}
+inline void cp_async_wait_all() { emu::drain_all_async(); }
 
 inline void prefetch_tensormap(const void *) {}
 inline void tma_load_2d(uint32_t dst, const void *map, int c0, int c1, uint32_t bar) {

@@ -38,7 +38,8 @@ def test_bench_cuda_arm_runs_end_to_end_on_tiny():
     assert j["n_gpus"] == 1 and j["steps"] == 2 and j["value"] > 0 and j["vs_baseline"] is None
     assert j["config"]["workload"] == "tiny" and j["config"]["w"] == 8
     assert j["config"]["kernel_variants"]["match"].startswith("cuda_core")
-    assert j["config"]["kernel_variants"]["selfcheck"]["slice_gcoop"] is True     # the classic warp-per-point slicer was checked in-process
+    sc = j["config"]["kernel_variants"]["selfcheck"]
+    assert sc["slice_gcoop"] is True and sc["slice_coop_ld"] is True          # the classic warp-per-point slicers were checked in-process
     assert j["roofline"]["bound"] in ("smem", "alu") and j["roofline"]["frac"] > 0
     assert j["kernels"]["match_prep"]["roofline"] is None          # CUDA-core matcher: no operand preparation
     assert j["gpu_launches"] == 2 * 6                               # 6 kernels of the library per step on the defaults
@@ -97,7 +98,7 @@ def test_gpu_variant_test_functions(gpu_tests):
     """tests/test_gpu_variants.py's own functions for the warp-per-point slicers and the tcgen05 matcher (tiny sizes)."""
     t, pkg, tiny = gpu_tests
     import test_gpu_variants as v
-    ok = {k: {"ok": True, "status": 0, "detail": ""} for k in ("slice_gcoop", "slice_coop", "match_cg1", "match_cg2")}
+    ok = {k: {"ok": True, "status": 0, "detail": ""} for k in ("slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2")}
     with dry_run():
         for name, impl in v.STAGED:
             v.test_staged_slice_tiny_full(pkg, tiny, ok, 0, True, name, impl)

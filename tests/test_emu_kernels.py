@@ -34,7 +34,7 @@ from emu_binding import EmuContext, EmuError, SPF_OUT_COMPLEX, SPF_OUT_INTENSITY
 SLICE_TOL = 1e-5
 DIST_TOL = 1e-4
 SLICERS = [(1, "thread-per-point global gather (library default)"), (3, "warp-per-point from global memory"),
-           (2, "warp-per-point from a TMA-staged tile")]
+           (4, "warp-per-point from a cp.async-staged tile"), (2, "warp-per-point from a TMA-staged tile")]
 MATCHERS = ["simt", "cg1", "cg2"]
 
 
@@ -109,11 +109,11 @@ def test_emulated_slice_tiny_vs_oracle(tiny, impl, what, force_complex, layout):
 
 
 def test_emulated_slicers_agree_bit_for_bit_where_they_should(tiny):
-    """Variants 2 and 3 walk the same window with the same weights in the same order: identical bits; and the result
+    """Variants 2, 3 and 4 walk the same window with the same weights in the same order: identical bits; and the result
     does not depend on how pixels are grouped into patches."""
     cfg, model, pix, refs, _ = tiny
     outs = {}
-    for impl in (2, 3):
+    for impl in (2, 3, 4):
         for layout in ((1, 32, 32), (4, 16, 16), (0, 0, 0)):
             ctx = EmuContext(cfg.N, eps=cfg.eps)
             ctx.set_detector_layout(*layout)
@@ -125,7 +125,7 @@ def test_emulated_slicers_agree_bit_for_bit_where_they_should(tiny):
         assert np.array_equal(v, first), k
 
 
-@pytest.mark.parametrize("impl", [1, 2, 3])
+@pytest.mark.parametrize("impl", [1, 2, 3, 4])
 @pytest.mark.parametrize("N,eps", [(16, 1e-6), (21, 1e-9), (12, 1e-4)])
 def test_emulated_slice_general_model_widths_and_even_n(impl, N, eps):
     """Non-even model (complex grid), even N, w = 8 / 10 / 6 (run-time width: reference gather only)."""
@@ -142,7 +142,7 @@ def test_emulated_slice_general_model_widths_and_even_n(impl, N, eps):
     assert _rel(c, orc.slice_points(A, refs, pix)) <= max(SLICE_TOL, 10 * eps)
 
 
-@pytest.mark.parametrize("impl", [1, 2, 3])
+@pytest.mark.parametrize("impl", [1, 2, 3, 4])
 def test_emulated_slice_edge_cases(tiny, impl):
     cfg, model, pix, refs, c_ref = tiny
     ctx = EmuContext(cfg.N, eps=cfg.eps)
@@ -277,7 +277,7 @@ def test_emulated_paper_scale_geometry_sampled(monkeypatch):
     sj = rng.integers(0, cfg.P, 1024)
     ref = orc.slice_points(model, refs, pix, np.zeros(1024, np.int64), sj)
     outs = {}
-    for impl in (1, 2):
+    for impl in (1, 2, 4):
         ctx.set_option("slice_impl", impl)
         eb.counters()
         outs[impl] = ctx.slice(refs, pix, SPF_OUT_COMPLEX)
@@ -287,7 +287,7 @@ def test_emulated_paper_scale_geometry_sampled(monkeypatch):
         assert err <= 2e-6
         if impl == 2:
             assert n["tma_copies"] >= 512 * 8                  # every one of the 512 blocks staged its box, >= 8 x-planes each
-    assert _rel(outs[2], outs[1]) <= 2e-6
+    assert _rel(outs[2], outs[1]) <= 2e-6 and np.array_equal(outs[4], outs[2])
 
 
 def test_emulated_spf_selftest_checks_and_switches_variants_on(tiny):
@@ -301,7 +301,7 @@ def test_emulated_spf_selftest_checks_and_switches_variants_on(tiny):
         ctx.selftest("slice_coop")
     assert e.value.status == -4                       # slicers check the caller's own model: SPF_ESTATE before prepare
     ctx.prepare_model(model)
-    for v in ("slice_gcoop", "slice_coop", "match_cg1", "match_cg2"):
+    for v in ("slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2"):
         r = ctx.selftest(v)
         print(v, r)
         assert r["passed"], r

@@ -44,14 +44,14 @@ def _require(verified, variant):
         pytest.fail("device self-check of %s did not pass (status %s): %s" % (variant, r["status"], r["detail"]))
 
 
-@pytest.mark.parametrize("variant", ["slice_gcoop", "slice_coop", "match_cg1", "match_cg2"])
+@pytest.mark.parametrize("variant", ["slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2"])
 def test_variant_selfcheck(verified, variant):
     _require(verified, variant)
 
 
 # --------------------------------------------------------------------------------- staged slicing
 
-STAGED = [("slice_gcoop", 3), ("slice_coop", 2)]
+STAGED = [("slice_gcoop", 3), ("slice_coop_ld", 4), ("slice_coop", 2)]
 
 
 @pytest.mark.parametrize("variant,impl", STAGED)
