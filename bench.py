@@ -249,7 +249,7 @@ def run_spf(args, cfg):
     # have been cleared on hardware: the default run never launches an unverified kernel.
     variants = (ctx.spf_autotune() if args.native else
                 {"slice_coop": False, "slice_gcoop": False, "slice_coop_ld": False, "match_cg1": False, "match_cg2": False,
-                 "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
+                 "match_mma": False, "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
     info = ctx.info
     measured = measure_device_peaks(ctx) if rank == 0 or world > 1 else {}
     d_model = torch.from_numpy(model).to(dev)
@@ -269,6 +269,12 @@ def run_spf(args, cfg):
             variants[v] = st["passed"]
             variants["slice_selftest"][v] = st["detail"]
         variants["slice_impl"] = ctx.spf_get_option("slice_impl")
+        # ... and the warp-level tensor-core matcher (mma.sync: classic CUDA too) against the CUDA-core reference; it replaces the
+        # CUDA-core matcher if it agrees.  The tcgen05 matcher is only reached with --native.
+        st = ctx.spf_selftest("match_mma")
+        variants["match_mma"] = st["passed"]
+        variants["match_selftest"] = st["detail"]
+        variants["match_impl"] = ctx.spf_get_option("match_impl")
     slices = ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=1.0)
     alpha = photon_scale(slices, mask, cfg.photons)
     images = torch.empty((cfg.n_img, cfg.P), dtype=torch.float32, device=dev)
@@ -350,7 +356,7 @@ def run_spf(args, cfg):
 
     peaks = _peaks()
     peaks.update(measured)
-    kern = roofline_objects(cfg, info, k_ms, products, peaks, clk)
+    kern = roofline_objects(cfg, info, k_ms, products, peaks, clk, "k_match_mma" if variants["match_impl"] == 2 else "k_match_gemm")
     dominant = max(("slice", "gemm"), key=lambda n: kern[n]["ms"])
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -363,7 +369,8 @@ def run_spf(args, cfg):
                                                      2: "tma_staged, warp per point", 3: "global_gather, warp per point",
                                                      4: "cp_async_staged, warp per point"}[variants["slice_impl"]],
                                            "match": ("tcgen05 cta_group::%d" % variants["match_cta_group"]) if variants["match_impl"] == 0
-                                                    else "cuda_core difference form (library default; tcgen05 variant %s)" % ("failed its self-check" if args.native else "not requested"),
+                                                    else ("mma.sync (legacy tensor-core path, classic CUDA; tcgen05 variant %s)" if variants["match_impl"] == 2
+                                                          else "cuda_core difference form (library default; tcgen05 variant %s)") % ("failed its self-check" if args.native else "not requested"),
                                            "selfcheck": variants},
                        "parallelism": "images partitioned x%d, orientations replicated" % world,
                        "l2": "inputs larger than L2 (slices %.2f GB, images %.2f GB per step; no flush needed)"
@@ -397,7 +404,7 @@ def run_spf(args, cfg):
         dist.destroy_process_group()
 
 
-def roofline_objects(cfg, info, k_ms, products, peaks, clk):
+def roofline_objects(cfg, info, k_ms, products, peaks, clk, tensor_kernel="k_match_gemm"):
     """Per-kernel roofline entries from the library's CUDA-event times.
 
     slice kernel: bound on chip -- every point needs w^3 grid values brought from shared memory to a lane
@@ -442,7 +449,7 @@ def roofline_objects(cfg, info, k_ms, products, peaks, clk):
         ach = products * alg / t_g / 1e12
         out["gemm"] = {"ms": t_g * 1e3, "products": products, "algorithmic_tflops_fp32_equivalent": alg / t_g / 1e12,
                        "images_per_s": cfg.n_img / t_g,
-                       "roofline": {"kernel": "k_match_gemm", "bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"],
+                       "roofline": {"kernel": tensor_kernel, "bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"],
                                     "unit": "TFLOP/s", "frac": ach / peaks["tensor_tflops"], "traffic": None,
                                     "peak_source": "%s sustained bf16 cuBLAS (fp16 = bf16 rate)" % peaks["source"]}}
     else:

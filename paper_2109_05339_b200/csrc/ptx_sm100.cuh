@@ -87,6 +87,30 @@ __device__ __forceinline__ void cp_async_16(uint32_t dst, const void *src) {
 // all cp.async of this thread issued so far have landed when this returns (other threads: follow with a block barrier)
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// 16 bytes, of which the first src_bytes (0 or 16) come from global memory and the rest are zero: rows past the end of a matrix
+__device__ __forceinline__ void cp_async_16_zfill(uint32_t dst, const void *src, uint32_t src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// at most N of this thread's committed groups are still in flight when this returns
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// ---------------------------------------------------------------- warp-level tensor-core path (mma.sync; SASS HMMA)
+// Four 8 x 8 matrices of 16-bit elements from shared memory: lane l supplies the address of row l % 8 of matrix l / 8
+// (16 bytes, 16-byte aligned); afterwards register j of lane l holds elements (row l / 4, columns 2 (l % 4), + 1) of matrix j.
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t row_addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(row_addr) : "memory");
+}
+// D (16 x 8, fp32) += A (16 x 16, fp16, row-major) * B (16 x 8, fp16, "column-major": 8 rows of 16 consecutive k).  With
+// g = lane / 4, t = lane % 4:  a0 = A[g][2t, 2t+1], a1 = A[g+8][2t, ..], a2 = A[g][2t+8, ..], a3 = A[g+8][2t+8, ..];
+// b0 = B[k = 2t, 2t+1][n = g], b1 = B[k = 2t+8, ..][g];  d0, d1 = D[g][2t, 2t+1], d2, d3 = D[g+8][2t, 2t+1].
+__device__ __forceinline__ void mma_m16n8k16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
 // ---------------------------------------------------------------- TMA
 __device__ __forceinline__ void prefetch_tensormap(const void *map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");

@@ -100,7 +100,7 @@ int spf_set_option(spf_ctx *ctx, const char *key, int64_t value) {
     if (!strcmp(key, "slice_impl") && value >= 1 && value <= 4) { ctx->opt_slice_impl = (int)value; return SPF_OK; }
     if (!strcmp(key, "force_complex_grid") && (value == 0 || value == 1)) { ctx->opt_force_complex = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_cta_group") && (value == 1 || value == 2)) { ctx->opt_match_cta_group = (int)value; return SPF_OK; }
-    if (!strcmp(key, "match_impl") && (value == 0 || value == 1)) { ctx->opt_match_impl = (int)value; return SPF_OK; }
+    if (!strcmp(key, "match_impl") && value >= 0 && value <= 2) { ctx->opt_match_impl = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_chunk_kblocks") && value >= 0 && value <= (1 << 20)) { ctx->opt_match_chunk_kb = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_condition") && (value == 0 || value == 1)) { ctx->opt_match_condition = (int)value; return SPF_OK; }
     if (!strcmp(key, "match_refine") && (value == 0 || value == 1)) { ctx->opt_match_refine = (int)value; return SPF_OK; }

@@ -502,6 +502,144 @@ k_match_simt(const float *__restrict__ images, int64_t n_img, const float *__res
 }
 
 // ------------------------------------------------------------------------------------------
+// Warp-level tensor-core matcher (option "match_impl" = 2): the same conditioned, split-precision contraction as
+// k_match_gemm -- same operand planes, same products, same fp64 epilogue, same packed-key argmin -- on the CLASSIC
+// CUDA tensor-core path: cp.async multi-stage pipeline, ldmatrix, mma.sync.m16n8k16 with fp32 accumulators in registers.
+// No tensor map, no mbarrier, no TMEM, no tcgen05: nothing in it that a device fault has ever been traced to, so it
+// can be checked in-process (spf_selftest "match_mma") and used where the tcgen05 kernel has not been cleared.  It is the
+// legacy path -- mma.sync cannot reach tcgen05 throughput on sm_100a -- and exists as the safe tensor-core matcher, not
+// as the product.  Block tile 128 images x 128 slices, 8 warps of 64 x 32, K stages of 32 pixels (64-byte rows, 16-byte
+// chunks XOR-swizzled with (row / 2) mod 4 so that ldmatrix reads 8 rows from 8 distinct bank groups).
+// ------------------------------------------------------------------------------------------
+constexpr int MM_BM = 128, MM_BN = 128, MM_BK = 32, MM_STAGES = 4, MM_THREADS = 256;
+constexpr int MM_TILE_BYTES = 128 * MM_BK * 2;   // 8 KB: 128 rows of 64 bytes
+template <int NI> struct MmaCfg {
+    static constexpr int TILES = NI + 2;          // image planes, then the two slice planes
+    static constexpr int STAGE_BYTES = TILES * MM_TILE_BYTES;
+    static constexpr int SMEM_BYTES = MM_STAGES * STAGE_BYTES;
+};
+__device__ __forceinline__ uint32_t mm_off(int row, int chunk) { return (uint32_t)(row * 64 + ((chunk ^ ((row >> 1) & 3)) << 4)); }
+
+template <int NI>
+__global__ void __launch_bounds__(MM_THREADS, 1)
+k_match_mma(const __half *__restrict__ plI, const __half *__restrict__ plS, int64_t Ppad, const MatchArgs a) {
+    using Cfg = MmaCfg<NI>;
+    if ((a.scal[2] != 0u) != (NI == 2)) return;   // the instantiation the data does not need
+    extern __shared__ __align__(128) uint8_t mm_smem[];
+    const uint32_t smem0 = ptx::smem_u32(mm_smem);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 2, wn = warp & 3;                       // warp grid 2 x 4: rows wm * 64, columns wn * 32
+    const int ib = (int)(blockIdx.x % (unsigned)a.n_ib), mb = (int)(blockIdx.x / (unsigned)a.n_ib);
+    const int64_t i0 = (int64_t)ib * MM_BM, m0 = (int64_t)mb * MM_BN;
+    const int nk = a.kblocks * (BK / MM_BK);                       // K steps of 32 pixels
+    const int chunk_steps = a.chunk_kb * (BK / MM_BK);
+
+    auto load_stage = [&](int kt, int slot) {
+        const uint32_t st = smem0 + (uint32_t)(slot * Cfg::STAGE_BYTES);
+        const int64_t k0 = (int64_t)kt * MM_BK;
+#pragma unroll
+        for (int it = 0; it < Cfg::TILES * 512 / MM_THREADS; ++it) {
+            const int idx = tid + it * MM_THREADS, tile = idx >> 9, r = (idx & 511) >> 2, c = idx & 3;
+            const bool img = tile < NI;
+            const int64_t rows = img ? a.n_img : a.M, row = (img ? i0 : m0) + r;
+            const int plane = img ? tile : tile - NI;
+            const __half *base = (img ? plI : plS) + (size_t)plane * (size_t)rows * (size_t)Ppad;
+            const int64_t rr = row < rows ? row : rows - 1;        // rows past the end: zero-filled, the address stays valid
+            ptx::cp_async_16_zfill(st + (uint32_t)(tile * MM_TILE_BYTES) + mm_off(r, c), base + rr * Ppad + k0 + c * 8, row < rows ? 16u : 0u);
+        }
+    };
+
+    float acc[4][4][4], tot[4][4][4];
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+#pragma unroll
+        for (int y = 0; y < 4; ++y)
+#pragma unroll
+            for (int z = 0; z < 4; ++z) acc[x][y][z] = tot[x][y][z] = 0.0f;
+
+    for (int s = 0; s < MM_STAGES - 1; ++s) {
+        if (s < nk) load_stage(s, s);
+        ptx::cp_async_commit();
+    }
+    int since_flush = 0;
+    for (int kt = 0; kt < nk; ++kt) {
+        ptx::cp_async_wait_group<MM_STAGES - 2>();   // stage kt has landed (this thread's pieces) ...
+        __syncthreads();                             // ... and everybody's; and every warp has finished stage kt - 1
+        if (kt + MM_STAGES - 1 < nk) load_stage(kt + MM_STAGES - 1, (kt + MM_STAGES - 1) % MM_STAGES);
+        ptx::cp_async_commit();
+        const uint32_t st = smem0 + (uint32_t)((kt % MM_STAGES) * Cfg::STAGE_BYTES);
+        const uint32_t tS1 = st + (uint32_t)(NI * MM_TILE_BYTES), tS2 = tS1 + MM_TILE_BYTES;
+#pragma unroll
+        for (int kk = 0; kk < MM_BK / 16; ++kk) {
+            uint32_t af[4][4], af2[4][4];
+            const int mat = lane >> 3, r8 = lane & 7;
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const int row = wm * 64 + mt * 16 + (mat & 1) * 8 + r8, chunk = kk * 2 + (mat >> 1);
+                ptx::ldmatrix_x4(af[mt], st + mm_off(row, chunk));
+                if (NI == 2) ptx::ldmatrix_x4(af2[mt], st + MM_TILE_BYTES + mm_off(row, chunk));
+            }
+#pragma unroll
+            for (int np = 0; np < 2; ++np) {          // pairs of 8-column tiles
+                uint32_t b1[4], b2[4];
+                const int n = wn * 32 + np * 16 + (mat >> 1) * 8 + r8, chunk = kk * 2 + (mat & 1);
+                ptx::ldmatrix_x4(b1, tS1 + mm_off(n, chunk));
+                ptx::ldmatrix_x4(b2, tS2 + mm_off(n, chunk));
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                    for (int nt = 0; nt < 2; ++nt) {
+                        ptx::mma_m16n8k16(acc[mt][np * 2 + nt], af[mt], b1[2 * nt], b1[2 * nt + 1]);            // I1 . S1
+                        ptx::mma_m16n8k16(acc[mt][np * 2 + nt], af[mt], b2[2 * nt], b2[2 * nt + 1]);            // I1 . S2
+                        if (NI == 2) ptx::mma_m16n8k16(acc[mt][np * 2 + nt], af2[mt], b1[2 * nt], b1[2 * nt + 1]);   // I2 . S1
+                    }
+            }
+        }
+        if (++since_flush == chunk_steps) {           // the chunk's sum joins the running total with round-to-nearest adds
+            since_flush = 0;
+#pragma unroll
+            for (int x = 0; x < 4; ++x)
+#pragma unroll
+                for (int y = 0; y < 4; ++y)
+#pragma unroll
+                    for (int z = 0; z < 4; ++z) { tot[x][y][z] += acc[x][y][z]; acc[x][y][z] = 0.0f; }
+        }
+    }
+    ptx::cp_async_wait_group<0>();
+
+    // epilogue: d = a_i + b_m - 2 G (fp64, rounded once), best of this thread's 8 columns per row, then of the 4 lanes that
+    // share the row; ascending column order and the packed key keep "lowest index wins ties"
+    const float neg2sc = spfmm::cross_scale((int)a.scal[4], (int)a.scal[5]);
+    const int g = lane >> 2, t = lane & 3;
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const int64_t i = i0 + wm * 64 + mt * 16 + g + 8 * half;
+            unsigned long long key = ~0ull;
+            if (i < a.n_img) {
+                const double aIv = a.aI[i];
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int64_t m = m0 + wn * 32 + nt * 8 + 2 * t + e;
+                        if (m < a.M) {
+                            const float G = tot[mt][nt][half * 2 + e] + acc[mt][nt][half * 2 + e];
+                            const unsigned long long k2 = spfmm::pack_key(spfmm::distance(aIv, __ldg(a.bS + m), neg2sc, G), a.m_base + (uint32_t)m);
+                            key = k2 < key ? k2 : key;
+                        }
+                    }
+            }
+            unsigned long long o = __shfl_xor_sync(0xffffffffu, key, 1);
+            key = o < key ? o : key;
+            o = __shfl_xor_sync(0xffffffffu, key, 2);
+            key = o < key ? o : key;
+            if (t == 0 && key != ~0ull) atomicMin(&a.keys[i], key);
+        }
+}
+
+// ------------------------------------------------------------------------------------------
 // reference matcher (tests only): difference form on the CUDA cores, fp64 accumulation
 // ------------------------------------------------------------------------------------------
 __global__ void k_match_ref_dist(const float *__restrict__ images, int64_t n_img, const float *__restrict__ slices, int64_t M,
@@ -640,6 +778,29 @@ static int match_pass(spf_ctx *ctx, const float *images, int64_t n_img, const fl
     k_split<<<(unsigned)M, 256, 0, st>>>(slices, P, L.Ppad, mask, cvec, scal, 1, M, plS, bS, nullptr);
     SPF_LAUNCH_CHECK(ctx);
 
+    if (ctx->opt_match_impl == 2) {
+        // the warp-level tensor-core matcher (mma.sync): same operand planes, one block per 128 x 128 tile, image tiles fastest
+        MatchArgs args{};
+        args.n_img = n_img; args.M = M; args.kblocks = (int)(L.Ppad / BK);
+        args.n_ib = (int)((n_img + MM_BM - 1) / MM_BM); args.n_mb = (int)((M + MM_BN - 1) / MM_BN);
+        args.m_base = (uint32_t)m_base;
+        args.chunk_kb = ctx->opt_match_chunk_kb > 0 ? ctx->opt_match_chunk_kb : args.kblocks;
+        args.keys = keys; args.aI = aI; args.bS = bS; args.scal = scal; args.fault = ctx->d_fault; args.abort_flag = ctx->d_abort;
+        if ((int64_t)args.n_ib * args.n_mb > 0x7fffffffLL) return spf_set_err(ctx, SPF_EINVAL, "spf_match: too many tiles");
+        const unsigned grid = (unsigned)(args.n_ib * args.n_mb);
+        auto mma1 = k_match_mma<1>, mma2 = k_match_mma<2>;
+        SPF_CUDA(ctx, cudaFuncSetAttribute(mma1, cudaFuncAttributeMaxDynamicSharedMemorySize, MmaCfg<1>::SMEM_BYTES));
+        SPF_CUDA(ctx, cudaFuncSetAttribute(mma2, cudaFuncAttributeMaxDynamicSharedMemorySize, MmaCfg<2>::SMEM_BYTES));
+        if ((rc = spf_record_event(ctx, 2, st))) return rc;
+        mma1<<<grid, MM_THREADS, MmaCfg<1>::SMEM_BYTES, st>>>(plI, plS, L.Ppad, args);
+        SPF_LAUNCH_CHECK(ctx);
+        mma2<<<grid, MM_THREADS, MmaCfg<2>::SMEM_BYTES, st>>>(plI, plS, L.Ppad, args);
+        SPF_LAUNCH_CHECK(ctx);
+        if ((rc = spf_record_event(ctx, 3, st))) return rc;
+        ctx->last_scal = scal; ctx->last_match_stream = st;
+        ctx->ev_valid[1] = ctx->ev_valid[2] = ctx->opt_record_events != 0;
+        return SPF_OK;
+    }
     const int CG = ctx->opt_match_cta_group;
     CUtensorMap a0, a1, b0, b1;
     if ((rc = encode_operand_map(ctx, &a0, plI, n_img, L.Ppad, TILE_ROWS))) return rc;
@@ -694,7 +855,7 @@ int spf_match(spf_ctx *ctx, const float *images, int64_t n_img, const float *sli
     unsigned long long *keys = (unsigned long long *)((uint8_t *)workspace + L.keys);
     k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
     SPF_LAUNCH_CHECK(ctx);
-    if (ctx->opt_match_impl == 0 && ctx->opt_match_refine) {
+    if (ctx->opt_match_impl != 1 && ctx->opt_match_refine) {
         k_match_refine<<<(unsigned)n_img, 256, 0, st>>>(images, slices, M, P, mask, best_idx, best_dist, 0);
         SPF_LAUNCH_CHECK(ctx);
     }
@@ -753,7 +914,7 @@ int spf_slice_match(spf_ctx *ctx, const float *quats, int64_t M, const float *pi
     unsigned long long *keys = (unsigned long long *)(ws + S.match.keys);
     k_match_finalize<<<(unsigned)((n_img + 255) / 256), 256, 0, st>>>(keys, n_img, best_idx, best_dist);
     SPF_LAUNCH_CHECK(ctx);
-    if (ctx->opt_match_impl == 0 && ctx->opt_match_refine) {
+    if (ctx->opt_match_impl != 1 && ctx->opt_match_refine) {
         // the winners' slices no longer exist: slice them again, chunk_M images at a time (n_img x P points in all)
         for (int64_t i0 = 0; i0 < n_img; i0 += chunk_M) {
             const int64_t nc = n_img - i0 < chunk_M ? n_img - i0 : chunk_M;

@@ -112,9 +112,10 @@ int selftest_slice(spf_ctx *ctx, int impl, spf_selftest_report *rep, cudaStream_
 // against spf_match_reference (difference form, fp64 accumulation).  With the refinement (the library's result): distances
 // within 1e-4 d.  Without it (the contraction's own a_i + b_m - 2 G): within 1e-4 d + 2e-6 of the norms, the expansion's
 // fp32 floor.  Argmin: equal, or the reference's own margin between the two candidates is inside that tolerance.
-int selftest_match(spf_ctx *ctx, int cta_group, spf_selftest_report *rep, cudaStream_t st) {
+int selftest_match(spf_ctx *ctx, int impl, int cta_group, spf_selftest_report *rep, cudaStream_t st) {
     const int keep[5] = {ctx->opt_match_impl, ctx->opt_match_cta_group, ctx->opt_match_refine, ctx->opt_record_events, ctx->last_match_impl};
-    ctx->opt_match_impl = 0; ctx->opt_match_cta_group = cta_group;
+    ctx->opt_match_impl = impl; ctx->opt_match_cta_group = cta_group;
+    const char *name = impl == 2 ? "mma.sync matcher" : (cta_group == 2 ? "tcgen05 matcher cta_group::2" : "tcgen05 matcher cta_group::1");
     struct Case { int n_img, M, P; bool counts; } cases[2] = {{300, 513, 2048, true}, {130, 257, 200, false}};
     if (ctx->opt_selftest_small) { cases[0] = Case{140, 18, 320, true}; cases[1] = Case{12, 260, 100, false}; }   // option "selftest_small"
     int rc = SPF_OK;
@@ -208,8 +209,8 @@ int selftest_match(spf_ctx *ctx, int cta_group, spf_selftest_report *rep, cudaSt
     ctx->last_scal = nullptr;   // the workspace of the check is gone
     if (rc != SPF_OK) return rc;
     rep->passed = ok; rep->worst_rel = worst; rep->ms_variant = ms_var; rep->ms_reference = ms_ref;
-    if (ok) say(rep, "tcgen05 matcher cta_group::%d vs CUDA-core reference: distances to %.1e, argmin equal outside near-ties", cta_group, worst);
-    else say(rep, "tcgen05 matcher cta_group::%d FAILED: %s", cta_group, why);
+    if (ok) say(rep, "%s vs CUDA-core reference: distances to %.1e, argmin equal outside near-ties, %.3f ms vs %.3f ms", name, worst, ms_var, ms_ref);
+    else say(rep, "%s FAILED: %s", name, why);
     return SPF_OK;
 }
 
@@ -231,14 +232,19 @@ extern "C" int spf_selftest(spf_ctx *ctx, const char *variant, spf_selftest_repo
         }
         return SPF_OK;
     }
+    if (!strcmp(variant, "match_mma")) {
+        if ((rc = selftest_match(ctx, 2, 1, report, st))) return rc;
+        if (report->passed && ctx->opt_match_impl == 1) ctx->opt_match_impl = 2;   // never replaces a verified tcgen05 matcher
+        return SPF_OK;
+    }
     if (!strcmp(variant, "match_cg1") || !strcmp(variant, "match_cg2")) {
         const int cg = variant[8] == '2' ? 2 : 1;
-        if ((rc = selftest_match(ctx, cg, report, st))) return rc;
+        if ((rc = selftest_match(ctx, 0, cg, report, st))) return rc;
         if (report->passed) {   // pairs supersede the single-CTA form; the single-CTA form never replaces verified pairs
-            if (ctx->opt_match_impl != 0 || cg == 2) ctx->opt_match_cta_group = cg;
+            if (ctx->opt_match_impl != 0 || cg == 2) ctx->opt_match_cta_group = cg;   // (also supersedes the mma.sync matcher)
             ctx->opt_match_impl = 0;
         }
         return SPF_OK;
     }
-    return spf_set_err(ctx, SPF_EINVAL, "spf_selftest: unknown variant %s (slice_gcoop, slice_coop_ld, slice_coop, match_cg1, match_cg2)", variant);
+    return spf_set_err(ctx, SPF_EINVAL, "spf_selftest: unknown variant %s (slice_gcoop, slice_coop_ld, slice_coop, match_mma, match_cg1, match_cg2)", variant);
 }

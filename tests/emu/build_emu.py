@@ -124,7 +124,7 @@ def build_emu(force: bool = False) -> str:
             fh.write(text)
     # the watchdog's bounds count emulator ticks (one per fiber switch), not SM clocks: keep them small so that a
     # pipeline that deadlocks under emulation reports SPF_EFAULT within seconds
-    flags = ["-O1", "-g", "-std=c++17", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing", "-DSPF_EMU", "-DSPF_DEBUG",
+    flags = ["-O2", "-g", "-std=c++17", "-fPIC", "-fvisibility=hidden", "-fno-strict-aliasing", "-DSPF_EMU", "-DSPF_DEBUG", "-U_FORTIFY_SOURCE", "-D_FORTIFY_SOURCE=0",
              "-DSPF_WAIT_CYCLES=(1ll<<22)", "-DSPF_DRAIN_CYCLES=(1ll<<8)", "-I" + HERE, "-I" + GEN, "-Wno-unused-value"]
     if asan:
         flags += ["-fsanitize=address", "-fno-omit-frame-pointer"]

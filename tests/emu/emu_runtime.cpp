@@ -1,6 +1,7 @@
 // tests/emu: scheduler, barriers, warp collectives, deferred asynchronous engines, shared-address map,
 // tensor-map encoder and the DFT behind the cuFFT stub.  See cuda_emu.h for the model.  TEST INFRASTRUCTURE ONLY.
 #include <stdarg.h>
+#include <setjmp.h>
 #include <ucontext.h>
 
 #include <deque>
@@ -17,8 +18,20 @@ double emu_now_ms() { return std::chrono::duration<double, std::milli>(std::chro
 
 namespace emu {
 
+// Fiber switches: a fiber is entered the first time with swapcontext (which installs its stack) and from then on with
+// _setjmp / _longjmp, which do not save the signal mask -- glibc's swapcontext makes a system call per switch, and the
+// emulator makes millions of switches.  Under AddressSanitizer (which tracks stacks through swapcontext) every switch
+// stays a swapcontext.
+#if defined(__SANITIZE_ADDRESS__)
+#define EMU_FAST_SWITCH 0
+#else
+#define EMU_FAST_SWITCH 1
+#endif
+
 struct Fiber {
     ucontext_t ctx;
+    jmp_buf jb;
+    bool started = false;
     char *stack = nullptr;
     bool done = true;
     int cta = 0, tid = 0;
@@ -35,6 +48,7 @@ long g_counters[4] = {0, 0, 0, 0};   // [0] bulk tensor copies, [1] tcgen05.mma,
 namespace {
 constexpr size_t STACK_BYTES = 256 * 1024;
 ucontext_t sched_ctx;
+jmp_buf sched_jb;
 std::vector<Fiber> fibers;
 std::vector<Cta> ctas;
 std::vector<uint8_t *> dyn_store;      // 1024-byte aligned, one per CTA of the cluster
@@ -65,7 +79,11 @@ void fiber_entry() {
     if (c.alive > 0 && c.bar_arrived == c.alive) { c.bar_arrived = 0; c.bar_gen++; }
     cluster_alive--;
     if (cluster_alive > 0 && cluster_arrived == cluster_alive) { cluster_arrived = 0; cluster_gen++; }
+#if EMU_FAST_SWITCH
+    _longjmp(sched_jb, 1);
+#else
     swapcontext(&f->ctx, &sched_ctx);
+#endif
 }
 
 void drain_async(bool all) {
@@ -95,7 +113,11 @@ void yield() {
     ++g_ticks;
     ++g_counters[3];
     Fiber *f = cur;
+#if EMU_FAST_SWITCH
+    if (!_setjmp(f->jb)) _longjmp(sched_jb, 1);
+#else
     swapcontext(&f->ctx, &sched_ctx);
+#endif
 }
 
 int cur_tid() { return cur->tid; }
@@ -199,7 +221,7 @@ void run_grid(dim3 grid, dim3 block, size_t dyn_bytes, int cluster, const std::f
             for (int w = 0; w < T / 32; ++w) c.warps[w].alive = 32;
             for (int t = 0; t < T; ++t) {
                 Fiber &f = fibers[(size_t)r * T + t];
-                f.done = false; f.cta = r; f.tid = t;
+                f.done = false; f.started = false; f.cta = r; f.tid = t;
                 f.t3 = dim3((unsigned)(t % block.x), (unsigned)((t / block.x) % block.y), (unsigned)(t / (block.x * block.y)));
                 getcontext(&f.ctx);
                 f.ctx.uc_stack.ss_sp = f.stack;
@@ -216,7 +238,15 @@ void run_grid(dim3 grid, dim3 block, size_t dyn_bytes, int cluster, const std::f
                 if (f.done) continue;
                 cur = &f; cur_cta = &ctas[(size_t)f.cta];
                 threadIdx = f.t3; blockIdx = cur_cta->bid;
+#if EMU_FAST_SWITCH
+                if (!_setjmp(sched_jb)) {
+                    if (f.started) _longjmp(f.jb, 1);
+                    f.started = true;
+                    swapcontext(&sched_ctx, &f.ctx);   // first entry: installs the fiber's stack (never returns here)
+                }
+#else
                 swapcontext(&sched_ctx, &f.ctx);
+#endif
                 if (!f.done) live++;
                 drain_async(false);
             }

@@ -68,6 +68,59 @@ inline void cp_async_16(uint32_t dst, const void *src) {
     emu::async_push([=]() { void *d = emu::shared_ptr(dst); if (d) memcpy(d, src, 16); });
 }
 inline void cp_async_wait_all() { emu::drain_all_async(); }
+inline void cp_async_16_zfill(uint32_t dst, const void *src, uint32_t src_bytes) {
+    if ((dst & 15u) || ((uintptr_t)src & 15u) || (src_bytes != 0u && src_bytes != 16u)) emu::fault("cp.async 16 (zfill %u): bad operands (shared 0x%x, global %p)", src_bytes, dst, src);
+    emu::async_push([=]() { uint8_t *d = (uint8_t *)emu::shared_ptr(dst); if (!d) return; memset(d, 0, 16); if (src_bytes) memcpy(d, src, src_bytes); });
+}
+inline void cp_async_commit() {}
+template <int N> inline void cp_async_wait_group() { emu::drain_all_async(); }   // a superset of what the hardware guarantees
+
+// ldmatrix / mma.sync: the fragment layouts of the PTX ISA, written out (the comments in ptx_sm100.cuh state them)
+inline void ldmatrix_x4(uint32_t (&r)[4], uint32_t row_addr) {
+    if (row_addr & 15u) emu::fault("ldmatrix: row address 0x%x not 16-byte aligned", row_addr);
+    const uint64_t *all = emu::warp_collective((uint64_t)row_addr);
+    const int lane = emu::lane();
+    for (int j = 0; j < 4; ++j) {
+        const uint8_t *row = (const uint8_t *)emu::shared_ptr((uint32_t)all[8 * j + (lane >> 2)]);
+        if (!row) { r[j] = 0xffffffffu; continue; }
+        memcpy(&r[j], row + 4 * (lane & 3), 4);
+    }
+    emu::warp_collective(0);   // nobody's deposited address is overwritten before everyone has read it
+}
+namespace emu_detail {
+inline float h2f(uint16_t h) {
+    const uint32_t sign = (uint32_t)(h & 0x8000u) << 16, e = (h >> 10) & 0x1fu, m = h & 0x3ffu;
+    uint32_t u;
+    if (e == 0) { const float sub = (float)m * 5.9604644775390625e-8f; return sign ? -sub : sub; }
+    if (e == 31) u = sign | 0x7f800000u | (m << 13); else u = sign | ((e + 112u) << 23) | (m << 13);
+    float f; memcpy(&f, &u, 4); return f;
+}
+}  // namespace emu_detail
+inline void mma_m16n8k16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    // three exchange rounds collect every lane's A and B registers; each lane then computes its own four outputs
+    uint32_t A[32][4], B[32][2];
+    const uint64_t *s = emu::warp_collective((uint64_t)a[0] | ((uint64_t)a[1] << 32));
+    for (int l = 0; l < 32; ++l) { A[l][0] = (uint32_t)s[l]; A[l][1] = (uint32_t)(s[l] >> 32); }
+    s = emu::warp_collective((uint64_t)a[2] | ((uint64_t)a[3] << 32));
+    for (int l = 0; l < 32; ++l) { A[l][2] = (uint32_t)s[l]; A[l][3] = (uint32_t)(s[l] >> 32); }
+    s = emu::warp_collective((uint64_t)b0 | ((uint64_t)b1 << 32));
+    for (int l = 0; l < 32; ++l) { B[l][0] = (uint32_t)s[l]; B[l][1] = (uint32_t)(s[l] >> 32); }
+    auto Ael = [&](int row, int k) {   // A[row][k], row < 16, k < 16
+        const int l = (row & 7) * 4 + ((k & 7) >> 1), reg = (row >> 3) + 2 * (k >> 3);
+        return emu_detail::h2f((uint16_t)(A[l][reg] >> (16 * (k & 1))));
+    };
+    auto Bel = [&](int k, int n) {     // B[k][n], k < 16, n < 8
+        const int l = n * 4 + ((k & 7) >> 1), reg = k >> 3;
+        return emu_detail::h2f((uint16_t)(B[l][reg] >> (16 * (k & 1))));
+    };
+    const int lane = emu::lane(), g = lane >> 2, t = lane & 3;
+    for (int o = 0; o < 4; ++o) {
+        const int row = g + 8 * (o >> 1), col = 2 * t + (o & 1);
+        float p = 0.0f;
+        for (int k = 0; k < 16; ++k) p += Ael(row, k) * Bel(k, col);
+        d[o] += p;
+    }
+}
 
 inline void prefetch_tensormap(const void *) {}
 inline void tma_load_2d(uint32_t dst, const void *map, int c0, int c1, uint32_t bar) {

@@ -65,4 +65,15 @@ def test_sass_uses_tcgen05_and_tma():
     sass = subprocess.run(["cuobjdump", "-sass", LIB_PATH], capture_output=True, text=True).stdout
     for mnemonic in ("UTCHMMA", "UTMALDG", "LDTM"):
         assert mnemonic in sass
-    assert "HMMA.16816" not in sass and "HGMMA" not in sass
+    assert "HGMMA" not in sass
+    # the legacy warp-level path (HMMA) exists in exactly one kernel family, the classic-CUDA matcher k_match_mma;
+    # the tcgen05 matcher and everything else carry none
+    per_fn = {}
+    name = None
+    for line in sass.splitlines():
+        if "Function :" in line:
+            name = line.split("Function :")[1].strip()
+        elif name and "HMMA" in line and "UTCHMMA" not in line:
+            per_fn[name] = per_fn.get(name, 0) + 1
+    assert per_fn and all("k_match_mma" in fn for fn in per_fn), sorted(per_fn)
+    assert any("UTCHMMA" in l for l in sass.splitlines())

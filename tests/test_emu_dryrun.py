@@ -19,6 +19,9 @@ sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
 sys.path.insert(0, os.path.join(ROOT, "tests"))
 from fake_cuda import dry_run  # noqa: E402
 
+FULL = os.environ.get("SPF_EMU_FULL", "0") == "1"      # default: one representative per code path; 1: every combination
+full_only = pytest.mark.skipif(not FULL, reason="SPF_EMU_FULL=1 runs every variant x case combination")
+
 
 def test_bench_cuda_arm_runs_end_to_end_on_tiny():
     """bench.py run_spf, config tiny, library defaults: warm-up, timed region, kernel-time pass, e2e through the
@@ -37,12 +40,13 @@ def test_bench_cuda_arm_runs_end_to_end_on_tiny():
         assert key in j, key
     assert j["n_gpus"] == 1 and j["steps"] == 2 and j["value"] > 0 and j["vs_baseline"] is None
     assert j["config"]["workload"] == "tiny" and j["config"]["w"] == 8
-    assert j["config"]["kernel_variants"]["match"].startswith("cuda_core")
+    assert j["config"]["kernel_variants"]["match"].startswith("mma.sync")    # the classic tensor-core matcher passed its in-process check
     sc = j["config"]["kernel_variants"]["selfcheck"]
-    assert sc["slice_gcoop"] is True and sc["slice_coop_ld"] is True          # the classic warp-per-point slicers were checked in-process
-    assert j["roofline"]["bound"] in ("smem", "alu") and j["roofline"]["frac"] > 0
-    assert j["kernels"]["match_prep"]["roofline"] is None          # CUDA-core matcher: no operand preparation
-    assert j["gpu_launches"] == 2 * 6                               # 6 kernels of the library per step on the defaults
+    assert sc["slice_gcoop"] is True and sc["slice_coop_ld"] is True and sc["match_mma"] is True          # the classic warp-per-point slicers were checked in-process
+    assert j["roofline"]["bound"] in ("smem", "tensor") and j["roofline"]["frac"] > 0
+    assert j["kernels"]["gemm"]["roofline"]["kernel"] == "k_match_mma" and j["kernels"]["gemm"]["products"] == 2
+    assert j["kernels"]["match_prep"]["roofline"]["bound"] == "hbm"
+    assert j["gpu_launches"] == 2 * 13                              # 3 prepare, 1 slice, 9 match (common vector, 2 abs-max, 2 split, 2 mma, finalize, refine)
     assert j["e2e"]["value"] > 0 and j["e2e"]["h2d_bytes_per_step"] > 16 * 1024 * 4 and j["e2e"]["d2h_bytes_per_step"] == 16 * 8
     assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["value"] > 0
     assert j["planted_hit_rate"] is not None
@@ -83,7 +87,7 @@ def test_gpu_parity_test_functions_prepare_and_slice(gpu_tests):
         t.test_slice_edge_cases(pkg, tiny)
 
 
-@pytest.mark.parametrize("variant", ["simt", "cg1", "cg2"])
+@pytest.mark.parametrize("variant", ["simt", pytest.param("mma", marks=full_only), pytest.param("cg1", marks=full_only), "cg2"])
 def test_gpu_parity_test_functions_match_and_end_to_end(gpu_tests, variant):
     t, pkg, tiny = gpu_tests
     with dry_run():
@@ -100,8 +104,26 @@ def test_gpu_variant_test_functions(gpu_tests):
     import test_gpu_variants as v
     ok = {k: {"ok": True, "status": 0, "detail": ""} for k in ("slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2")}
     with dry_run():
-        for name, impl in v.STAGED:
+        for name, impl in (v.STAGED if FULL else v.STAGED[-1:]):
             v.test_staged_slice_tiny_full(pkg, tiny, ok, 0, True, name, impl)
             v.test_staged_slice_general_model(pkg, ok, 16, 1e-6, name, impl)
         v.test_staged_slice_equals_the_layout_free_result(pkg, tiny, ok)
         v.test_tcgen05_end_to_end_tiny(pkg, tiny, ok)
+
+
+def test_gpu_classic_variant_test_functions(gpu_tests):
+    """tests/test_gpu_parity_classic_variants.py's own functions (the default-on GPU tests of slice_impl 3 / 4 and the
+    mma.sync matcher), tiny sizes."""
+    t, pkg, tiny = gpu_tests
+    import test_gpu_parity_classic_variants as c
+    with dry_run():
+        for impl in (c.CLASSIC_SLICERS if FULL else c.CLASSIC_SLICERS[-1:]):
+            c.test_classic_slice_tiny_full(pkg, tiny, impl, 0, True)
+            c.test_classic_slice_general_model(pkg, impl, 16, 1e-6)
+            if FULL:
+                c.test_classic_slice_tiny_full(pkg, tiny, impl, 1, False)
+                c.test_classic_slice_general_model(pkg, impl, 21, 1e-9)
+        c.test_mma_match_vs_oracle_ragged_sizes(pkg, 16, 64, 1024, False)
+        if FULL:
+            c.test_mma_match_vs_oracle_ragged_sizes(pkg, 5, 300, 1000, True)
+            c.test_mma_match_planted_ties_and_general_values(pkg)

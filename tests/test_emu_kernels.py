@@ -33,9 +33,13 @@ from emu_binding import EmuContext, EmuError, SPF_OUT_COMPLEX, SPF_OUT_INTENSITY
 
 SLICE_TOL = 1e-5
 DIST_TOL = 1e-4
+# The default run (a few minutes, what `pytest -m "not gpu"` executes) keeps one representative of every kernel and code
+# path; SPF_EMU_FULL=1 adds every (variant x case) combination (about ten minutes).
+FULL = os.environ.get("SPF_EMU_FULL", "0") == "1"
+full_only = pytest.mark.skipif(not FULL, reason="SPF_EMU_FULL=1 runs every variant x case combination")
 SLICERS = [(1, "thread-per-point global gather (library default)"), (3, "warp-per-point from global memory"),
            (4, "warp-per-point from a cp.async-staged tile"), (2, "warp-per-point from a TMA-staged tile")]
-MATCHERS = ["simt", "cg1", "cg2"]
+MATCHERS = ["simt", "mma", "cg1", "cg2"]
 
 
 def _rel(a, b):
@@ -52,7 +56,7 @@ def tiny():
 
 
 def _matcher(ctx, variant):
-    ctx.set_option("match_impl", 1 if variant == "simt" else 0)
+    ctx.set_option("match_impl", {"simt": 1, "mma": 2}.get(variant, 0))
     ctx.set_option("match_cta_group", 2 if variant == "cg2" else 1)
 
 
@@ -167,7 +171,8 @@ def test_emulated_slice_edge_cases(tiny, impl):
 # --------------------------------------------------------------------------------- a6-a8: spf_match
 
 @pytest.mark.parametrize("variant", MATCHERS)
-@pytest.mark.parametrize("n_img,M,P,masked", [(16, 64, 1024, False), (5, 300, 1000, True), (130, 257, 192, False), (300, 513, 320, True)])
+@pytest.mark.parametrize("n_img,M,P,masked", [(16, 64, 1024, False), (5, 300, 1000, True), (130, 257, 192, False),
+                                              pytest.param(300, 513, 320, True, marks=full_only)])
 def test_emulated_match_vs_oracle_ragged_sizes(variant, n_img, M, P, masked):
     rng = np.random.default_rng(n_img * 7 + M)
     S = (rng.random((M, P)) * rng.random((M, 1)) * 3).astype(np.float32)
@@ -179,7 +184,8 @@ def test_emulated_match_vs_oracle_ragged_sizes(variant, n_img, M, P, masked):
     bi, bd, prods = ctx.match(I, S, mask)
     n = eb.counters()
     assert prods == (0 if variant == "simt" else 2)              # photon counts: one fp16 image plane
-    assert (n["mmas"] > 0) == (variant != "simt") and (n["tma_copies"] > 0) == (variant != "simt")
+    tc = variant in ("cg1", "cg2")                                # only the tcgen05 matcher issues tcgen05.mma and bulk tensor copies
+    assert (n["mmas"] > 0) == tc and (n["tma_copies"] > 0) == tc
     _check_match(bi, bd, I, S, mask)
     if n_img * M <= 2000:                                        # the independent CUDA-core reference kernels (one block per
         ri, rd, dist = ctx.match_reference(I, S, mask)           # pair: only the small cases are affordable under emulation)
@@ -187,7 +193,7 @@ def test_emulated_match_vs_oracle_ragged_sizes(variant, n_img, M, P, masked):
         assert np.array_equal(ri, bi) or variant != "simt"
 
 
-@pytest.mark.parametrize("variant", ["cg1", "cg2"])
+@pytest.mark.parametrize("variant", ["mma", "cg1", "cg2"])
 @pytest.mark.parametrize("chunk", [1, 3, 0])
 def test_emulated_tcgen05_epilogue_without_refinement(variant, chunk):
     """The contraction's own a_i + b_m - 2 G (match_refine = 0), with the accumulator drained every 1 or 3 K blocks
@@ -236,7 +242,8 @@ def test_emulated_match_planted_ties_and_general_values(variant):
 
 # --------------------------------------------------------------------------------- the whole path
 
-@pytest.mark.parametrize("impl,variant", [(1, "simt"), (3, "simt"), (2, "cg1"), (2, "cg2")])
+@pytest.mark.parametrize("impl,variant", [(1, "simt"), pytest.param(3, "simt", marks=full_only), (4, "mma"),
+                                          pytest.param(2, "cg1", marks=full_only), (2, "cg2")])
 def test_emulated_end_to_end_tiny_poisson(tiny, impl, variant):
     """Tiny (BASELINE.json:configs[0]) end to end: everything from the oracle on one side, everything from the
     emulated kernels on the other -- the library defaults, and the TMA-staged slicer with each tcgen05 matcher."""
@@ -301,7 +308,7 @@ def test_emulated_spf_selftest_checks_and_switches_variants_on(tiny):
         ctx.selftest("slice_coop")
     assert e.value.status == -4                       # slicers check the caller's own model: SPF_ESTATE before prepare
     ctx.prepare_model(model)
-    for v in ("slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2"):
+    for v in (("slice_gcoop", "slice_coop_ld", "slice_coop", "match_mma", "match_cg1", "match_cg2") if FULL else ("slice_coop_ld", "slice_coop", "match_cg2")):
         r = ctx.selftest(v)
         print(v, r)
         assert r["passed"], r
@@ -318,7 +325,8 @@ def test_emulated_spf_selftest_checks_and_switches_variants_on(tiny):
     _check_match(bi, bd, I, S)
 
 
-@pytest.mark.parametrize("impl,variant", [(1, "simt"), (2, "cg1"), (2, "cg2")])
+@pytest.mark.parametrize("impl,variant", [(1, "simt"), pytest.param(4, "mma", marks=full_only),
+                                          pytest.param(2, "cg1", marks=full_only), (2, "cg2")])
 def test_emulated_streaming_slice_match_equals_the_two_step_path(tiny, impl, variant):
     """spf_slice_match: 64 orientations in ragged chunks of 24 -- the slice array never exists -- give
     the argmin and distances of spf_slice + spf_match, and agree with the oracle end to end."""

@@ -233,8 +233,9 @@ def test_match_vs_oracle_ragged_sizes(spf, n_img, M, P, masked):
 
 
 def set_match_variant(ctx, variant):
-    """"simt": the CUDA-core matcher (library default); "cg1" / "cg2": the tcgen05 GEMM on single CTAs / CTA pairs."""
-    ctx.spf_set_option("match_impl", 1 if variant == "simt" else 0)
+    """"simt": the CUDA-core matcher (library default); "mma": the warp-level tensor-core matcher (mma.sync);
+    "cg1" / "cg2": the tcgen05 GEMM on single CTAs / CTA pairs."""
+    ctx.spf_set_option("match_impl", {"simt": 1, "mma": 2}.get(variant, 0))
     ctx.spf_set_option("match_cta_group", 2 if variant == "cg2" else 1)
 
 
