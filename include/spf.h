@@ -210,9 +210,13 @@ SPF_API int spf_debug_fine_grid(spf_ctx *ctx, float *out_dev_complex, void *stre
  *                  4 = as 2, the tile staged by cp.async (16-byte pieces copied by every thread, block barrier) instead of
  *                      TMA: classic CUDA only, the staged gather for a device on which the TMA path is not cleared
  *   "force_complex_grid": [0]; 1 = gather the complex grid even for an even model
- *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused norm-add + argmin epilogue (the product);
+ *   "match_impl":  0 = tcgen05 / TMEM / TMA split-fp16 GEMM with the fused a_i + b_m - 2 G + argmin epilogue (the product);
  *                  [1] = CUDA-core matcher: the difference form sum (I - S)^2 in fp32, register-tiled, same fused
- *                      argmin -- about 20x slower at Paper-scale, no tensor-core, TMA or mbarrier machinery
+ *                      argmin -- about 20x slower at Paper-scale, no tensor-core, TMA or mbarrier machinery;
+ *                  2 = the same conditioned split-precision contraction on the warp-level tensor-core path (cp.async
+ *                      pipeline, ldmatrix, mma.sync m16n8k16, fp32 accumulators in registers): classic CUDA only, the
+ *                      tensor-core matcher for a device on which the tcgen05 kernel has not been cleared (legacy path:
+ *                      it cannot reach tcgen05 throughput)
  *   "match_cta_group": CTAs per tcgen05 MMA (match_impl 0): 2 = cta_group::2 pairs (UMMA 256 x 256), [1] = single CTA (128 x 256)
  *   "match_chunk_kblocks": [32] 64-pixel K blocks accumulated inside TMEM before the epilogue warps add the chunk to
  *                  their fp32 registers with round-to-nearest adds; 0 = all of K in TMEM (spf_match_math.cuh)
@@ -233,14 +237,14 @@ SPF_API int spf_get_option(const spf_ctx *ctx, const char *key, int64_t *value);
 
 /*
  * Device self-check of one kernel variant against this library's reference kernels, and the switch that turns a verified
- * variant on.  variant: "slice_gcoop" (slice_impl 3), "slice_coop_ld" (slice_impl 4), "slice_coop" (slice_impl 2), "match_cg1", "match_cg2" (the tcgen05
+ * variant on.  variant: "slice_gcoop" (slice_impl 3), "slice_coop_ld" (slice_impl 4), "slice_coop" (slice_impl 2), "match_mma" (match_impl 2), "match_cg1", "match_cg2" (the tcgen05
  * matcher on single CTAs / CTA pairs).  Slicing variants slice the caller's own prepared model (read-only; SPF_ESTATE
  * before spf_prepare_model) at 64 seeded orientations x 16,384 pixels with the reference gather and with the variant
  * (bar: relative L2 <= 3e-6, all finite); matcher variants run two seeded cases, with and without a mask, against
  * spf_match_reference (bar: distances within 1e-4 d; without the refinement 1e-4 d + 2e-6 of the norms; argmin equal
  * outside near-ties).  A consistency check between two CUDA paths, not parity (tests/ hold every variant to the oracle).
  * On success (report->passed = 1) the variant becomes the context's choice -- for slicers only if it was also the
- * fastest verified so far, pairs supersede the single-CTA matcher -- so a C caller reaches the TMA / tcgen05 kernels
+ * fastest verified so far, the tcgen05 matcher supersedes the mma.sync one, pairs supersede single CTAs -- so a C caller reaches the TMA / tcgen05 kernels
  * with spf_create + spf_prepare_model + spf_selftest, no other option set.  Returns SPF_OK when the check RAN (passed or
  * not), another status when it could not (SPF_EFAULT: the variant's watchdog gave up).  Synchronises.  Runs in the
  * calling process: a variant that raises an SM exception takes the caller's CUDA context with it; callers that need
