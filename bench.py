@@ -247,9 +247,7 @@ def run_spf(args, cfg):
     # kernel variants: the library defaults, or with --native the faster ones (TMA-staged gather, tcgen05 GEMM) whose
     # device self-check passes in a child process (paper_2109_05339_b200/selfcheck.py).  Opt-in until those kernels
     # have been cleared on hardware: the default run never launches an unverified kernel.
-    variants = (ctx.spf_autotune() if args.native else
-                {"slice_coop": False, "slice_gcoop": False, "slice_coop_ld": False, "match_cg1": False, "match_cg2": False,
-                 "match_mma": False, "slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "native": "off (run with --native to self-check and use them)"})
+    variants = {"slice_impl": 1, "match_impl": 1, "match_cta_group": 1, "tier": "reference kernels"}
     info = ctx.info
     measured = measure_device_peaks(ctx) if rank == 0 or world > 1 else {}
     d_model = torch.from_numpy(model).to(dev)
@@ -259,22 +257,13 @@ def run_spf(args, cfg):
     # workload generation (outside every timed region): Poisson means come from the CUDA slicer at the
     # truth orientations -- inputs, not a correctness reference
     ctx.spf_prepare_model(d_model)
-    if not args.native and not args.reference_kernels_only:
-        # Among the CLASSIC-CUDA slicers (no TMA, mbarrier or tcgen05 in either) the C library checks the warp-per-point
-        # gather against the reference gather on this model and switches it on if it agrees and is faster (spf_selftest).
-        # (3: straight from global memory; 4: from a tile staged by cp.async).  The fastest one that agrees is used.
-        variants["slice_selftest"] = {}
-        for v in ("slice_gcoop", "slice_coop_ld"):
-            st = ctx.spf_selftest(v)
-            variants[v] = st["passed"]
-            variants["slice_selftest"][v] = st["detail"]
-        variants["slice_impl"] = ctx.spf_get_option("slice_impl")
-        # ... and the warp-level tensor-core matcher (mma.sync: classic CUDA too) against the CUDA-core reference; it replaces the
-        # CUDA-core matcher if it agrees.  The tcgen05 matcher is only reached with --native.
-        st = ctx.spf_selftest("match_mma")
-        variants["match_mma"] = st["passed"]
-        variants["match_selftest"] = st["detail"]
-        variants["match_impl"] = ctx.spf_get_option("match_impl")
+    # Kernel variants.  Default: the classic-CUDA fast tier (warp-per-point slicers from global memory / from a cp.async-staged
+    # tile, the mma.sync matcher -- no tensor map, mbarrier, TMEM or tcgen05 in any of them).  --native adds the TMA-staged slicer
+    # and the tcgen05 matcher (opt-in until cleared on hardware).  Either way every candidate is checked by
+    # the C library's spf_selftest in a CHILD process first and switched on only if it agrees with the reference kernels.
+    if not args.reference_kernels_only:
+        variants = ctx.spf_autotune(classic_only=not args.native)
+        variants["tier"] = "classic + TMA / tcgen05 (--native)" if args.native else "classic CUDA (default)"
     slices = ctx.spf_slice(d_refs, d_pix, SPF_OUT_INTENSITY, scale=1.0)
     alpha = photon_scale(slices, mask, cfg.photons)
     images = torch.empty((cfg.n_img, cfg.P), dtype=torch.float32, device=dev)

@@ -180,22 +180,33 @@ class SpfContext:
         return {"passed": bool(rep.passed), "ms_variant": float(rep.ms_variant), "ms_reference": float(rep.ms_reference),
                 "worst_rel": float(rep.worst_rel), "detail": rep.detail.decode(errors="replace")}
 
-    def spf_autotune(self, timeout_s: float = 240.0) -> dict:
-        """Switch on the faster kernel variants that pass the device self-check (selfcheck.py, run once per
-        process in a child process so that a faulting variant cannot take this process's CUDA context with
-        it): for slicing the verified variant that the check timed fastest (one warp per point, TMA-staged
-        or straight from global memory), for matching the tcgen05 GEMM (cta_group::2 when verified, else single CTA),
-        else the CUDA-core matcher stays.  Returns {variant: bool} plus "slice_impl" / "match_impl" /
-        "match_cta_group" = the options now in force."""
-        from .selfcheck import verified_variants, fastest_slice_impl
+    def spf_autotune(self, timeout_s: float = 240.0, classic_only: bool = False) -> dict:
+        """Switch on the faster kernel variants that pass the library's own device check.  Each variant's check
+        (spf_selftest, C) first runs in a CHILD process (selfcheck.py), least machinery first, stopping at the first child
+        that dies -- a faulting variant cannot take this process's CUDA context with it; for every variant whose child
+        passed, spf_selftest is then called on THIS context, which is what switches it on (the C library keeps the
+        fastest verified slicer; tcgen05 supersedes mma.sync, CTA pairs supersede single CTAs).  classic_only=True limits the
+        candidates to the classic-CUDA tier (slice_impl 3 / 4, match_impl 2): no tensor map, mbarrier, TMEM or tcgen05.
+        The model must be prepared (the slicing checks slice the caller's own model).  Returns {variant: bool} plus
+        "slice_impl" / "match_impl" / "match_cta_group" = the options now in force, and "detail" per variant."""
+        from .selfcheck import verified_variants, CLASSIC
         report = {}
-        ok = dict(verified_variants(self.device.index or 0, timeout_s, report))
-        ok["slice_impl"] = fastest_slice_impl(report)
-        ok["match_cta_group"] = 2 if ok.get("match_cg2") else 1
-        ok["match_impl"] = 0 if (ok.get("match_cg1") or ok.get("match_cg2")) else 1
-        self.spf_set_option("match_impl", ok["match_impl"])
-        self.spf_set_option("slice_impl", ok["slice_impl"])
-        self.spf_set_option("match_cta_group", ok["match_cta_group"])
+        ok = dict(verified_variants(self.device.index or 0, timeout_s, report, only=CLASSIC if classic_only else None))
+        ok["detail"] = {}
+        for v, passed in list(ok.items()):
+            if v == "detail":
+                continue
+            if passed and v.startswith("slice") and not self.info.prepared:
+                ok[v] = False
+                ok["detail"][v] = "not switched on: the slicing checks slice the caller's model (call spf_prepare_model first)"
+            elif passed:
+                st = self.spf_selftest(v)
+                ok[v] = st["passed"]
+                ok["detail"][v] = st["detail"]
+            else:
+                ok["detail"][v] = "child check: " + str((report.get(v) or {}).get("detail", ""))[:160]
+        for k in ("slice_impl", "match_impl", "match_cta_group"):
+            ok[k] = self.spf_get_option(k)
         return ok
 
     def spf_launch_count(self) -> int:

@@ -34,7 +34,8 @@ import sys
 import time
 
 # least machinery first: classic CUDA (no TMA / mbarrier / tcgen05), then TMA + mbarrier, then tcgen05, CTA pairs last
-VARIANTS = ("slice_gcoop", "slice_coop_ld", "slice_coop", "match_cg1", "match_cg2")
+VARIANTS = ("slice_gcoop", "slice_coop_ld", "match_mma", "slice_coop", "match_cg1", "match_cg2")
+CLASSIC = ("slice_gcoop", "slice_coop_ld", "match_mma")      # classic CUDA only: no tensor map, mbarrier, TMEM or tcgen05
 SLICE_IMPL = {"slice_coop": 2, "slice_gcoop": 3, "slice_coop_ld": 4}
 _ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 _cache = {}
@@ -89,7 +90,7 @@ def run_variant(variant: str, device: int = 0):
     """Returns (one-line description, metrics dict)."""
     if variant in SLICE_IMPL:
         return _check_slice(device, variant)
-    if variant in ("match_cg1", "match_cg2"):
+    if variant in ("match_mma", "match_cg1", "match_cg2"):
         return _check_match(device, variant), {}
     raise ValueError("unknown variant %r (one of %s)" % (variant, ", ".join(VARIANTS)))
 
@@ -156,9 +157,9 @@ def _disk_cache_path(device: int) -> str:
     return os.path.join(where, "libspf_selfcheck_%s_%s.json" % (h, uuid.replace("/", "_")))
 
 
-def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = None) -> dict:
-    """{variant: passed} for every variant, each checked once per library build and GPU (cached in the
-    process and on disk)."""
+def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = None, only=None) -> dict:
+    """{variant: passed} for every variant (or for the subset `only`, in VARIANTS order), each checked once per
+    library build and GPU (cached in the process and on disk)."""
     path = _disk_cache_path(device)
     disk = {}
     if path and os.path.exists(path):
@@ -169,7 +170,7 @@ def verified_variants(device: int = 0, timeout_s: float = 240.0, report: dict = 
             disk = {}
     out = {}
     stopped_by = None
-    for v in VARIANTS:
+    for v in (VARIANTS if only is None else [x for x in VARIANTS if x in only]):
         key = (v, device)
         if key not in _cache:
             if stopped_by is not None:

@@ -102,7 +102,16 @@ def dry_run(sm_count=4):
         self.spf_set_option("selftest_small", 1)
         return saved["microbench"](self, what)
 
+    import paper_2109_05339_b200.selfcheck as sc
+    saved["child"], saved["cache_env"] = sc.check_in_child, os.environ.get("SPF_SELFCHECK_CACHE")
+
+    def _child_ok(variant, device=0, timeout_s=240.0):   # there is no device for a child process to check: pretend it passed
+        return {"ok": True, "status": 0, "kind": "agrees", "detail": "dry run: child check skipped", "seconds": 0.0, "metrics": {}}
+
     try:
+        sc.check_in_child = _child_ok
+        sc._cache.clear()
+        os.environ["SPF_SELFCHECK_CACHE"] = "off"
         b.SpfContext.spf_selftest, b.SpfContext.spf_microbench = _selftest_small, _microbench_small
         b.LIB_PATH, b._lib = build_emu(), None
         b._dev, b._stream, b.torch = _dev, (lambda device: None), proxy
@@ -115,6 +124,12 @@ def dry_run(sm_count=4):
         real_torch.Tensor.to = _to
         yield proxy
     finally:
+        sc.check_in_child = saved["child"]
+        sc._cache.clear()
+        if saved["cache_env"] is None:
+            os.environ.pop("SPF_SELFCHECK_CACHE", None)
+        else:
+            os.environ["SPF_SELFCHECK_CACHE"] = saved["cache_env"]
         b.SpfContext.spf_selftest, b.SpfContext.spf_microbench = saved["selftest"], saved["microbench"]
         b.LIB_PATH, b._lib, b._dev, b._stream, b.torch = saved["lib_path"], saved["lib"], saved["dev"], saved["stream"], saved["btorch"]
         sys.modules["torch"] = saved["sys_torch"]

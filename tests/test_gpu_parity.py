@@ -357,9 +357,9 @@ def test_paper_scale_sampled(spf):
     refs = random_quaternions(cfg.M, seed=2)
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    variants = choose_variants(ctx)   # what bench.py does: defaults, or (opt-in) the variants the device self-check passes
-    print("paper-scale runs with", variants)
     ctx.spf_prepare_model(_dev(model))
+    variants = choose_variants(ctx)   # defaults, or (opt-in) the variants the device self-check passes; after prepare: the slicing checks use the model
+    print("paper-scale runs with", variants)
     c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX)
     sm, sj = sample_pairs(cfg.M, cfg.P, 4096)
     got = c[torch.from_numpy(sm).cuda(), torch.from_numpy(sj).cuda()].cpu().numpy()

@@ -35,8 +35,8 @@ def test_slicing_heavy_sampled(spf):
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
     assert ctx.info.w == 10
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    print("slicing-heavy runs with", choose_variants(ctx))
     ctx.spf_prepare_model(_dev(model))
+    print("slicing-heavy runs with", choose_variants(ctx))
     assert ctx.info.grid_is_real == 1
     sm, sj = sample_pairs(cfg.M, cfg.P, 2048)
     got = np.empty(len(sm), np.complex64)
@@ -108,8 +108,8 @@ def test_streaming_equals_two_step_on_small(spf):
     refs = random_quaternions(cfg.M, seed=2)
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    print("streaming (small) runs with", choose_variants(ctx))
     ctx.spf_prepare_model(_dev(model))
+    print("streaming (small) runs with", choose_variants(ctx))
     d_refs, d_pix = _dev(refs), _dev(pix)
     slices = ctx.spf_slice(d_refs, d_pix, spf.SPF_OUT_INTENSITY, scale=1.0)
     alpha = photon_scale(slices, None, cfg.photons)
@@ -139,8 +139,8 @@ def test_paper_shaped_streaming_sampled(spf):
     refs = random_quaternions(cfg.M, seed=2)
     ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
     ctx.spf_set_detector_layout(cfg.panels, cfg.panel_edge, cfg.panel_edge)
-    print("paper-shaped runs with", choose_variants(ctx))
     ctx.spf_prepare_model(_dev(model))
+    print("paper-shaped runs with", choose_variants(ctx))
     d_refs, d_pix, d_mask = _dev(refs), _dev(pix), _dev(mask)
     rng = np.random.default_rng(7)
     planted = rng.integers(0, cfg.M, cfg.n_img)
