@@ -119,20 +119,6 @@ def check_in_child(variant: str, device: int = 0, timeout_s: float = 240.0) -> d
             "seconds": round(time.time() - t0, 1), "metrics": metrics}
 
 
-def fastest_slice_impl(report: dict) -> int:
-    """slice_impl to use given a verified_variants report: the verified variant with the lowest timed
-    spf_slice, provided it beat the global gather in its own child's timing; else 1 (global gather)."""
-    best, best_ms = 1, None
-    for v, impl in SLICE_IMPL.items():
-        r = report.get(v) or {}
-        m = r.get("metrics") or {}
-        if not r.get("ok") or "slice_ms" not in m:
-            continue
-        if m["slice_ms"] < m.get("slice_ms_global", float("inf")) and (best_ms is None or m["slice_ms"] < best_ms):
-            best, best_ms = impl, m["slice_ms"]
-    return best
-
-
 def _disk_cache_path(device: int) -> str:
     """One file per (library build, GPU) under <repository>/gpurun_out/selfcheck/: a later PROCESS of the same
     job reuses the verdicts instead of launching a variant that already faulted once more (every bench /

@@ -126,16 +126,3 @@ def test_reference_arm_other_ranks_exit_without_work():
     p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "tiny",
                         "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
     assert p.returncode == 0 and p.stdout.strip() == ""
-
-
-def test_autotune_picks_the_fastest_verified_slicing_variant():
-    """selfcheck.fastest_slice_impl: only variants whose child check passed AND beat the global gather in that
-    child's own timing are eligible; the lowest time wins; otherwise the library default (1) stays."""
-    from paper_2109_05339_b200.selfcheck import fastest_slice_impl
-    ok = lambda ms, g=10.0: {"ok": True, "metrics": {"slice_ms": ms, "slice_ms_global": g}}
-    assert fastest_slice_impl({}) == 1
-    assert fastest_slice_impl({"slice_gcoop": ok(5.0), "slice_coop": ok(3.0)}) == 2
-    assert fastest_slice_impl({"slice_gcoop": ok(2.0), "slice_coop": ok(3.0)}) == 3
-    assert fastest_slice_impl({"slice_gcoop": ok(12.0), "slice_coop": {"ok": False, "metrics": {"slice_ms": 1.0}}}) == 1
-    assert fastest_slice_impl({"slice_coop": {"ok": True, "metrics": {}}}) == 1
-    assert fastest_slice_impl({"slice_gcoop": ok(4.0), "slice_coop": ok(6.0)}) == 3

@@ -102,3 +102,28 @@ def test_mma_match_paper_scale_sampled(spf):
     sel = torch.from_numpy(rows).cuda()
     ties = base._check_match(bi[sel], bd[sel], images[sel].cpu().numpy(), S.cpu().numpy(), mask, "paper-scale mma")
     print("paper-scale, mma.sync matcher: 24 sampled rows agree with the oracle (%d near-ties)" % ties)
+
+
+def test_selftest_switches_the_classic_variants_on_in_process(spf, tiny):
+    """spf_selftest (the C library's own check) on the device: the classic variants agree with the reference kernels and
+    become the context's choice -- what bench.py relies on."""
+    cfg, model, pix, refs, c_ref = tiny
+    ctx = spf.SpfContext(cfg.N, eps=cfg.eps)
+    ctx.spf_prepare_model(_dev(model))
+    for v in ("slice_gcoop", "slice_coop_ld", "match_mma"):
+        r = ctx.spf_selftest(v)
+        print(v, r["detail"])
+        assert r["passed"], r
+    assert ctx.spf_get_option("match_impl") == 2 and ctx.spf_get_option("slice_impl") in (1, 3, 4)
+    c = ctx.spf_slice(_dev(refs), _dev(pix), spf.SPF_OUT_COMPLEX).cpu().numpy()     # whatever is now switched on still matches the oracle
+    assert _rel_l2(c, c_ref) <= SLICE_TOL
+
+
+def test_microbench_reports_device_figures(spf):
+    """spf_microbench: the SM-side denominators bench.py measures before its timed region.  Loose sanity bounds only (the
+    figures themselves are the measurement): every one is finite and above what any working B200 delivers."""
+    ctx = spf.SpfContext(8)
+    got = {k: ctx.spf_microbench(k) for k in ("lds32", "lds128", "l2", "hbm_copy")}
+    print("spf_microbench GB/s:", {k: round(v, 1) for k, v in got.items()})
+    assert got["lds32"] > 2000 and got["lds128"] > 2000 and got["l2"] > 1000 and got["hbm_copy"] > 1000
+    assert all(np.isfinite(v) and v < 1e6 for v in got.values())
