@@ -19,8 +19,8 @@ sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
 sys.path.insert(0, os.path.join(ROOT, "tests"))
 from fake_cuda import dry_run  # noqa: E402
 
-FULL = os.environ.get("SPF_EMU_FULL", "0") == "1"      # default: one representative per code path; 1: every combination
-full_only = pytest.mark.skipif(not FULL, reason="SPF_EMU_FULL=1 runs every variant x case combination")
+FULL = os.environ.get("SPF_EMU_FULL", "1") == "1"      # default: every combination; 0: one representative per code path
+full_only = pytest.mark.skipif(not FULL, reason="SPF_EMU_FULL=0: one representative per code path")
 
 
 def test_bench_cuda_arm_runs_end_to_end_on_tiny():

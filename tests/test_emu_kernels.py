@@ -33,10 +33,10 @@ from emu_binding import EmuContext, EmuError, SPF_OUT_COMPLEX, SPF_OUT_INTENSITY
 
 SLICE_TOL = 1e-5
 DIST_TOL = 1e-4
-# The default run (a few minutes, what `pytest -m "not gpu"` executes) keeps one representative of every kernel and code
-# path; SPF_EMU_FULL=1 adds every (variant x case) combination (about ten minutes).
-FULL = os.environ.get("SPF_EMU_FULL", "0") == "1"
-full_only = pytest.mark.skipif(not FULL, reason="SPF_EMU_FULL=1 runs every variant x case combination")
+# Every (variant x case) combination runs by default (under three minutes); SPF_EMU_FULL=0 keeps one representative of
+# every kernel and code path (for the AddressSanitizer build, which is several times slower).
+FULL = os.environ.get("SPF_EMU_FULL", "1") == "1"
+full_only = pytest.mark.skipif(not FULL, reason="SPF_EMU_FULL=0: one representative per code path")
 SLICERS = [(1, "thread-per-point global gather (library default)"), (3, "warp-per-point from global memory"),
            (4, "warp-per-point from a cp.async-staged tile"), (2, "warp-per-point from a TMA-staged tile")]
 MATCHERS = ["simt", "mma", "cg1", "cg2"]
