@@ -20,8 +20,9 @@ GEN = os.path.join(HERE, "gen")
 LIB = os.path.join(HERE, "libspf_emu.so")
 SOURCES = ["spf_api.cu", "spf_prepare.cu", "spf_slice.cu", "spf_match.cu", "spf_selftest.cu", "spf_microbench.cu"]
 HEADERS = ["spf_internal.cuh", "ptx_sm100.cuh", "spf_slice_math.cuh", "spf_match_math.cuh"]
-EMU_FILES = ["cuda_emu.h", "ptx_emu.cuh", "emu_runtime.cpp", "build_emu.py", os.path.join("selftest", "emu_faults.cu")]
-EXTRA = [os.path.join(HERE, "selftest", "emu_faults.cu")]     # deliberately broken kernels: the emulator's own self-test
+EMU_FILES = ["cuda_emu.h", "ptx_emu.cuh", "emu_runtime.cpp", "build_emu.py", os.path.join("selftest", "emu_faults.cu"), os.path.join("selftest", "emu_probes.cu")]
+# the emulator's own self-test: deliberately broken kernels, and one-instruction probes compared with CuTe's tables
+EXTRA = [os.path.join(HERE, "selftest", "emu_faults.cu"), os.path.join(HERE, "selftest", "emu_probes.cu")]
 
 
 def _match_close(text, start, open_ch, close_ch):
