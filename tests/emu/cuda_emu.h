@@ -101,6 +101,11 @@ const char *last_fault();                                 // non-empty after an 
 void fault(const char *fmt, ...);
 void clear_fault();
 extern long g_counters[4];
+// shared-memory wavefront accounting of the 16-byte-granular instructions (a MODEL: 8 x 16-byte bank groups per 128-byte
+// wavefront, a warp-wide access served quarter-warp by quarter-warp, equal addresses merged)
+extern long g_smem_counters[4];      // [0] ldmatrix 8-row phases, [1] wavefronts they take, [2] cp.async.16 quarter-warp groups, [3] wavefronts
+void note_ldmatrix(const uint64_t *addr32);
+void note_cp_async16(uint32_t dst);
 
 template <class... KA, class... A>
 void launch(void (*kern)(KA...), dim3 grid, dim3 block, size_t dyn_smem, int cluster, A &&...a) {

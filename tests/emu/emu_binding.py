@@ -77,6 +77,15 @@ def counters(reset=True):
     return {"tma_copies": out[0], "mmas": out[1], "launches": out[2], "fiber_switches": out[3]}
 
 
+def smem_counters(reset=True):
+    """Shared-memory wavefront accounting of the 16-byte-granular instructions since the last reset (a MODEL: 8 bank groups
+    of 16 bytes per wavefront, warp-wide accesses served quarter-warp by quarter-warp, equal addresses merged):
+    ldmatrix 8-row phases / the wavefronts they take, cp.async.16 quarter-warp groups / the wavefronts they take."""
+    out = (C.c_long * 4)()
+    lib().spf_emu_smem_counters(out, int(reset))
+    return {"ldsm_phases": out[0], "ldsm_wavefronts": out[1], "cpasync_groups": out[2], "cpasync_wavefronts": out[3]}
+
+
 def _p(a):
     return C.c_void_p(a.ctypes.data) if a is not None else None
 

@@ -4,6 +4,7 @@
 #include <setjmp.h>
 #include <ucontext.h>
 
+#include <array>
 #include <deque>
 #include <string>
 #include <vector>
@@ -35,6 +36,7 @@ struct Fiber {
     char *stack = nullptr;
     bool done = true;
     int cta = 0, tid = 0;
+    long cp_seq = 0;          // how many cp.async.16 this thread has issued in this block (lanes of a warp issue them in step)
     dim3 t3;
 };
 
@@ -43,6 +45,7 @@ Cta *cur_cta = nullptr;
 int g_cluster_size = 1;
 long long g_ticks = 0;
 int g_sm_count = 4;
+long g_smem_counters[4] = {0, 0, 0, 0};
 long g_counters[4] = {0, 0, 0, 0};   // [0] bulk tensor copies, [1] tcgen05.mma, [2] kernel launches, [3] fiber switches
 
 namespace {
@@ -63,6 +66,34 @@ uint32_t rng_state = 12345u;
 std::vector<const void *> static_shared;   // static __shared__ objects whose address was taken (mbarriers of k_slice)
 constexpr uint32_t WINDOW = 0x00000400u;     // shared-window offset of the dynamic block inside a CTA (1024-aligned, keeps addresses < 256 KB)
 constexpr uint32_t STATIC_BASE = 0x00800000u;
+
+// cp.async.16 destinations of the running block: [cta * 32 + warp][sequence number][lane] (0 = no access)
+std::vector<std::vector<std::array<uint32_t, 32>>> cp_log;
+
+// wavefronts a group of up to 8 sixteen-byte accesses takes: the busiest of the 8 bank groups, equal addresses merged
+int wavefronts16(const uint32_t *addr, int n) {
+    int worst = 0;
+    for (int g = 0; g < 8; ++g) {
+        uint32_t seen[8]; int ns = 0;
+        for (int i = 0; i < n; ++i) {
+            if (!addr[i] || (int)((addr[i] >> 4) & 7u) != g) continue;
+            bool dup = false;
+            for (int k = 0; k < ns; ++k) dup = dup || seen[k] == addr[i];
+            if (!dup) seen[ns++] = addr[i];
+        }
+        worst = ns > worst ? ns : worst;
+    }
+    return worst;
+}
+void flush_cp_log() {
+    for (auto &w : cp_log)
+        for (auto &ins : w)
+            for (int q = 0; q < 4; ++q) {
+                const int wf = wavefronts16(&ins[(size_t)q * 8], 8);
+                if (wf) { g_smem_counters[2]++; g_smem_counters[3] += wf; }
+            }
+    cp_log.clear();
+}
 
 uint32_t rnd() { rng_state = rng_state * 1664525u + 1013904223u; return rng_state >> 8; }
 
@@ -121,6 +152,21 @@ void yield() {
 }
 
 int cur_tid() { return cur->tid; }
+void note_ldmatrix(const uint64_t *addr32) {
+    for (int j = 0; j < 4; ++j) {
+        uint32_t a[8];
+        for (int i = 0; i < 8; ++i) a[i] = (uint32_t)addr32[8 * j + i] | 0x80000000u;    // never 0 ("no access")
+        g_smem_counters[0]++;
+        g_smem_counters[1] += wavefronts16(a, 8);
+    }
+}
+void note_cp_async16(uint32_t dst) {
+    const size_t w = (size_t)cur->cta * 32 + (size_t)(cur->tid >> 5);
+    if (cp_log.size() <= w) cp_log.resize(w + 1);
+    const size_t seq = (size_t)cur->cp_seq++;
+    if (cp_log[w].size() <= seq) cp_log[w].resize(seq + 1, std::array<uint32_t, 32>{});
+    cp_log[w][seq][(size_t)(cur->tid & 31)] = dst | 0x80000000u;
+}
 Cta *cta_of_rank(int rank) {
     if (rank < 0 || rank >= (int)ctas.size()) { fault("CTA rank %d outside the cluster of %zu", rank, ctas.size()); return &ctas[0]; }
     return &ctas[rank];
@@ -221,7 +267,7 @@ void run_grid(dim3 grid, dim3 block, size_t dyn_bytes, int cluster, const std::f
             for (int w = 0; w < T / 32; ++w) c.warps[w].alive = 32;
             for (int t = 0; t < T; ++t) {
                 Fiber &f = fibers[(size_t)r * T + t];
-                f.done = false; f.started = false; f.cta = r; f.tid = t;
+                f.done = false; f.started = false; f.cta = r; f.tid = t; f.cp_seq = 0;
                 f.t3 = dim3((unsigned)(t % block.x), (unsigned)((t / block.x) % block.y), (unsigned)(t / (block.x * block.y)));
                 getcontext(&f.ctx);
                 f.ctx.uc_stack.ss_sp = f.stack;
@@ -252,6 +298,7 @@ void run_grid(dim3 grid, dim3 block, size_t dyn_bytes, int cluster, const std::f
             }
         }
         drain_async(true);
+        flush_cp_log();
         for (int r = 0; r < cluster; ++r)
             if (ctas[(size_t)r].tmem_cols != 0) fault("block %ld exited with %d TMEM columns still allocated", b0 + r, ctas[(size_t)r].tmem_cols);
     }
@@ -457,6 +504,9 @@ extern "C" {
 __attribute__((visibility("default"))) const char *spf_emu_last_fault(void) { return emu::last_fault(); }
 __attribute__((visibility("default"))) void spf_emu_counters(long *out4, int reset) {
     for (int i = 0; i < 4; ++i) { out4[i] = emu::g_counters[i]; if (reset) emu::g_counters[i] = 0; }
+}
+__attribute__((visibility("default"))) void spf_emu_smem_counters(long *out4, int reset) {
+    for (int i = 0; i < 4; ++i) { out4[i] = emu::g_smem_counters[i]; if (reset) emu::g_smem_counters[i] = 0; }
 }
 __attribute__((visibility("default"))) void spf_emu_clear_fault(void) { emu::clear_fault(); }
 __attribute__((visibility("default"))) void spf_emu_set_sm_count(int n) { emu::g_sm_count = n > 0 ? n : 1; }

@@ -65,11 +65,13 @@ inline bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 // cp.async: deferred like every other asynchronous copy; wait_all drains the queue (all threads' copies: a superset)
 inline void cp_async_16(uint32_t dst, const void *src) {
     if ((dst & 15u) || ((uintptr_t)src & 15u)) emu::fault("cp.async 16: unaligned address (shared 0x%x, global %p)", dst, src);
+    emu::note_cp_async16(dst);
     emu::async_push([=]() { void *d = emu::shared_ptr(dst); if (d) memcpy(d, src, 16); });
 }
 inline void cp_async_wait_all() { emu::drain_all_async(); }
 inline void cp_async_16_zfill(uint32_t dst, const void *src, uint32_t src_bytes) {
     if ((dst & 15u) || ((uintptr_t)src & 15u) || (src_bytes != 0u && src_bytes != 16u)) emu::fault("cp.async 16 (zfill %u): bad operands (shared 0x%x, global %p)", src_bytes, dst, src);
+    emu::note_cp_async16(dst);
     emu::async_push([=]() { uint8_t *d = (uint8_t *)emu::shared_ptr(dst); if (!d) return; memset(d, 0, 16); if (src_bytes) memcpy(d, src, src_bytes); });
 }
 inline void cp_async_commit() {}
@@ -80,6 +82,7 @@ inline void ldmatrix_x4(uint32_t (&r)[4], uint32_t row_addr) {
     if (row_addr & 15u) emu::fault("ldmatrix: row address 0x%x not 16-byte aligned", row_addr);
     const uint64_t *all = emu::warp_collective((uint64_t)row_addr);
     const int lane = emu::lane();
+    if (lane == 0) emu::note_ldmatrix(all);
     for (int j = 0; j < 4; ++j) {
         const uint8_t *row = (const uint8_t *)emu::shared_ptr((uint32_t)all[8 * j + (lane >> 2)]);
         if (!row) { r[j] = 0xffffffffu; continue; }

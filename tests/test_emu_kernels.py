@@ -102,9 +102,11 @@ def test_emulated_slice_tiny_vs_oracle(tiny, impl, what, force_complex, layout):
     ctx.set_option("slice_impl", impl)
     ctx.set_option("force_complex_grid", force_complex)
     ctx.prepare_model(model)
-    eb.counters()
+    eb.counters(); eb.smem_counters()
     c = ctx.slice(refs[:m], pix, SPF_OUT_COMPLEX)
-    n = eb.counters()
+    n, sm = eb.counters(), eb.smem_counters()
+    # the cp.async-staged tile (impl 4) is written one shared-memory wavefront per quarter-warp (the emulator's bank model)
+    assert (sm["cpasync_groups"] > 0) == (impl == 4) and sm["cpasync_wavefronts"] == sm["cpasync_groups"], sm
     assert np.isfinite(c.view(np.float32)).all()
     assert _rel(c, c_ref[:m]) <= SLICE_TOL
     assert (n["tma_copies"] > 0) == (impl == 2), n          # the staged variant really stages, the others never touch TMA
@@ -191,6 +193,28 @@ def test_emulated_match_vs_oracle_ragged_sizes(variant, n_img, M, P, masked):
         ri, rd, dist = ctx.match_reference(I, S, mask)           # pair: only the small cases are affordable under emulation)
         assert np.allclose(dist, orc.distances(I, S, mask), rtol=1e-6)
         assert np.array_equal(ri, bi) or variant != "simt"
+
+
+def test_emulated_mma_matcher_shared_memory_accesses_are_conflict_free():
+    """k_match_mma's XOR swizzle (chunk ^ (row / 2) mod 4 over 64-byte rows): every ldmatrix phase (8 rows of 16 bytes)
+    and every quarter-warp of cp.async.16 stores touches 8 distinct 16-byte bank groups, i.e. takes ONE shared-memory
+    wavefront -- counted from the addresses the kernel's own source produces, for the one-plane and the two-plane
+    (non-integer images) instantiation.  A model of the bank rule, not a hardware counter."""
+    rng = np.random.default_rng(5)
+    for integer_images in (True, False):
+        S = (rng.random((140, 320)) * 3).astype(np.float32)
+        I = rng.poisson(S[rng.integers(0, 140, 130)]).astype(np.float32)
+        if not integer_images:
+            I = I + rng.random(I.shape).astype(np.float32)
+        ctx = EmuContext(8, sm_count=4)
+        _matcher(ctx, "mma")
+        eb.smem_counters()
+        bi, bd, prods = ctx.match(I, S, None)
+        n = eb.smem_counters()
+        assert prods == (2 if integer_images else 3)
+        assert n["ldsm_phases"] > 0 and n["ldsm_wavefronts"] == n["ldsm_phases"], n
+        assert n["cpasync_groups"] > 0 and n["cpasync_wavefronts"] == n["cpasync_groups"], n
+        _check_match(bi, bd, I, S, None)
 
 
 @pytest.mark.parametrize("variant", ["mma", "cg1", "cg2"])
